@@ -1,0 +1,137 @@
+/* include/vr.h — C ABI of the B200 ray-casting volume renderer (libvr_b200.so).
+ *
+ * The hot path of Hassan, Fluke & Barnes, "Interactive Visualization of the Largest
+ * Radioastronomy Cubes": ray casting of a float32 spectral cube that is
+ * partitioned object-wise into bricks (section 2.3), one image per brick inside
+ * its "rendering rectangle" (section 2.4), then depth-ordered sort-last
+ * composition of the brick images into one frame (section 2.5).  The paper
+ * states the problem as "cube of floats + colour map + transformation/projection matrices in,
+ * W x H frame out" and gives no formulas; the formulas are the readings
+ * O1-O11 / A1-A16 of DESIGN.md ("Readings of the paper").
+ *
+ * Pointer convention: names starting with d_ are DEVICE pointers owned by the caller (e.g.
+ * torch-allocated); every other pointer is HOST memory.  No torch types cross this boundary.
+ * All work is enqueued on the volume's stream (vr_set_stream; default = legacy stream 0) and the
+ * calls return without synchronising unless stated.  Every call returns a vr_status; the message
+ * for the last failure on the calling thread is vr_last_error().  Nothing throws or aborts.
+ * There is NO CPU fallback: without a CUDA device every compute call returns VR_ERR_CUDA.
+ *
+ * Geometry conventions (O1-O3, O11):
+ *   cube       float32, dims (nx,ny,nz), x fastest: data[(z*ny + y)*nx + x]; voxel (i,j,k) is the
+ *              unit cell [i,i+1)x[j,j+1)x[k,k+1) with its value at the cell centre; the volume
+ *              box is [0,nx]x[0,ny]x[0,nz] in voxel units.
+ *   image      float32 RGBA, row-major [py][px][4]; py = 0 is the BOTTOM row; rays go through
+ *              pixel centres; emission-absorption colours are premultiplied by alpha; pixels
+ *              whose ray misses the volume are (0,0,0,0).
+ */
+#ifndef VR_H
+#define VR_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct vr_volume vr_volume; /* opaque: owns the tiled copy, the tables, the brick images */
+
+typedef enum {
+    VR_OK = 0,
+    VR_ERR_INVALID_ARG = 1, /* NULL pointer, non-positive size, non-finite value, bad enum ...  */
+    VR_ERR_STATE = 2,       /* e.g. render before a transfer function was set                   */
+    VR_ERR_OOM = 3,         /* device allocation failed                                         */
+    VR_ERR_CUDA = 4         /* CUDA runtime failure (no device, launch error ...)               */
+} vr_status;
+
+typedef enum { VR_MODE_EA = 0, VR_MODE_MIP = 1 } vr_mode;     /* PAPER.md:80 / PAPER.md:150    */
+typedef enum { VR_PROJ_ORTHO = 0, VR_PROJ_PERSP = 1 } vr_proj;
+
+/* The "transformation and projection matrices" the viewer sends per frame. */
+typedef struct {
+    float view[16];     /* row-major 4x4, voxel space -> eye space, rigid (rotation+translation);
+                           the eye looks down -z_eye, +x_eye is right, +y_eye is up             */
+    int   projection;   /* vr_proj                                                              */
+    float fovy_deg;     /* PERSP: full vertical field of view, in (0,180)                       */
+    float ortho_half_h; /* ORTHO: half height of the view window in voxels (half width = *W/H)  */
+} vr_camera;
+
+#define VR_MAX_BRICKS 512 /* bx*by*bz */
+
+/* a0  Brick partitioner / tiled re-layout ("loads its portion").
+ *     Copies the linear cube d_data[nz][ny][nx] into the library's own tiled layout (8x8x8-voxel
+ *     tiles, edge-replicated padding) with one streaming kernel.
+ *     d_data is read during the call only (the call synchronises the stream before returning, so
+ *     the caller may free d_data afterwards).  Allocates ~1.01x the cube on the device.
+ *     INVALID_ARG: NULL, dim <= 0, dim > 65528.  OOM / CUDA on failure.                         */
+vr_status vr_create_volume(const int dims[3] /* nx,ny,nz */, const float* d_data, vr_volume** out);
+void      vr_destroy_volume(vr_volume* vol);
+
+/* Stream for all later work of this volume (a cudaStream_t passed as void*). */
+vr_status vr_set_stream(vr_volume* vol, void* cuda_stream);
+
+/* Colour map ("transfer function"; PAPER.md:138 colour map sent by the viewer).
+ *     rgba: 256 entries (r,g,b,a) in [0,1], un-premultiplied, HOST; entry j sits at data value
+ *     vmin + (vmax-vmin)*j/255; values between entries are linearly interpolated, values outside
+ *     [vmin,vmax] clamp (O6).  Alpha is opacity per voxel of path length; each render
+ *     corrects it per entry for its step: 1-(1-a)^step.  INVALID_ARG: NULL, vmax <= vmin,
+ *     non-finite, entry outside [0,1].                                                          */
+vr_status vr_set_transfer_function(vr_volume* vol, const float rgba[256 * 4], float vmin, float vmax);
+
+/* Object-space partition into bx*by*bz bricks with faces at floor(m*n_a/b_a) (
+ *     DESIGN.md O9/A10).  Default 1,1,1.  INVALID_ARG: b_a < 1, b_a > n_a, product > VR_MAX_BRICKS. */
+vr_status vr_set_bricks(vr_volume* vol, int bx, int by, int bz);
+
+/* a1-a7  One frame: per-brick ray casting inside each brick's rendering rectangle
+ *     (PAPER.md:150), then depth-ordered composition into d_out_rgba.
+ *     step_voxels: sampling distance along the ray in voxels, > 0.
+ *     mode: VR_MODE_EA (front-to-back emission-absorption) or VR_MODE_MIP (maximum intensity,
+ *           colour-mapped at the end, un-premultiplied).
+ *     ert_alpha: early ray termination (Levoy 1990) when a brick's accumulated
+ *           opacity reaches this value; <= 0 or >= 1 disables it.  Ignored for MIP.
+ *     d_out_rgba: DEVICE, H*W*4 floats.  d_out_scalar: DEVICE, H*W floats or NULL; MIP only:
+ *           the raw maximum per pixel ("2D floating point array of maximum recorded
+ *           scalar value"), -inf where the ray takes no sample.
+ *     INVALID_ARG: NULL, W/H <= 0 or > 32768, step <= 0 or non-finite, unknown mode/projection,
+ *     view not rigid within 1e-4, fovy outside (0,180), ortho_half_h <= 0.  STATE: no transfer
+ *     function yet.  Asynchronous on the stream (first use at a new image size allocates).      */
+vr_status vr_render(vr_volume* vol, const vr_camera* cam, int W, int H, float step_voxels, int mode,
+                    float ert_alpha, float* d_out_rgba, float* d_out_scalar);
+
+/* Same frame delivered to HOST memory: vr_render into an internal device frame, then a
+ *     device->host copy of it into h_out_rgba (H*W*4 floats; pinned memory makes the copy
+ *     asynchronous) and a stream synchronisation.  This is the end-to-end call bench.py times. */
+vr_status vr_render_to_host(vr_volume* vol, const vr_camera* cam, int W, int H, float step_voxels,
+                            int mode, float ert_alpha, float* h_out_rgba);
+
+/* Inspection level (the paper's two stages taken apart):
+ * vr_render_bricks: steps a1-a5 only.  d_brick_images: DEVICE, caller-owned, B*H*W*4 floats (EA:
+ *     premultiplied C_b, A_b) or B*H*W floats (MIP: M_b, -inf = no sample), full frames, brick
+ *     index b = (bk*by + bj)*bx + bi; pixels outside a brick's rectangle are 0 / -inf.
+ * vr_composite: steps a6-a7 on such a stack of brick images.                                    */
+vr_status vr_render_bricks(vr_volume* vol, const vr_camera* cam, int W, int H, float step_voxels,
+                           int mode, float ert_alpha, float* d_brick_images);
+vr_status vr_composite(vr_volume* vol, const vr_camera* cam, int W, int H, int mode,
+                       const float* d_brick_images, float* d_out_rgba, float* d_out_scalar);
+
+/* Host-only planning step (a2 rendering rectangles, a6 depth order), no device needed:
+ *     out_rect[b] = {x0, y0, w, h} of brick b's rendering rectangle (w = 0: off-screen),
+ *     out_order[k] = brick index of the k-th brick front to back (A11, A12).         */
+vr_status vr_plan_bricks(const int dims[3], const int bricks[3], const vr_camera* cam, int W, int H,
+                         int out_rect[][4], int out_order[]);
+
+/* Measurement aids (not on the product path):
+ * vr_measure: renders the frame with the instrumented build of the caster and returns, in HOST
+ *     counters, the samples actually evaluated and the number of distinct 32-byte sectors of the
+ *     tiled cube that the samples' 2x2x2 footprints touched (algorithmic HBM bytes = 32 * that).
+ *     Synchronises.  Either output may be NULL.                                                  */
+vr_status vr_measure(vr_volume* vol, const vr_camera* cam, int W, int H, float step_voxels, int mode,
+                     float ert_alpha, long long* h_samples, long long* h_sectors);
+/* Device time of the re-layout kernel of vr_create_volume, in ms, and the bytes it allocated.  */
+vr_status vr_volume_info(const vr_volume* vol, float* h_relayout_ms, long long* h_tiled_bytes);
+/* Inverse of the re-layout: gathers the tiled copy back into d_linear[nz][ny][nx] (round-trip test). */
+vr_status vr_export_linear(vr_volume* vol, float* d_linear);
+
+const char* vr_last_error(void); /* thread-local, never NULL */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VR_H */

@@ -1,0 +1,410 @@
+// kernels.cuh — the sm_100a kernels of the hot path.
+//
+//   relayout_kernel   a0  linear cube -> 8x8x8-voxel tiles
+//   cast_kernel<EA>   a1,a3,a4  per-brick ray caster, emission-absorption
+//   cast_kernel<MIP>  a1,a3,a5  maximum-intensity variant
+//   composite_kernel  a7  depth-ordered "over" / max of the brick images
+//
+// Per-ray set-up (ray, slab clips, sample index ranges) is double precision and follows DESIGN.md
+// O2-O4 and O9 term by term; per-sample work is fp32.  No code is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace vr {
+
+constexpr int TILE = 8;                 // voxels per tile edge
+constexpr int TILE_ELEMS = 512;         // 8^3 floats = 2 KB, x-rows of 32 B = one DRAM sector
+constexpr int CTA_PX = 16;              // a CTA renders a 16x16-pixel tile: 8 warps of 8x4 pixels
+constexpr int CTA_THREADS = 256;
+constexpr int MODE_EA = 0, MODE_MIP = 1;
+
+struct FrameParams {
+    double eye[3], right[3], up[3], fwd[3];   // O1
+    double h, asp, tanhalf;                   // O2: ortho half height, W/H, tan(fovy/2)
+    double step;                              // O4: Delta in voxels
+    int proj, W, H;
+    int nx, ny, nz;
+    unsigned ty_stride;                       // elements between tiles adjacent in y  = TX*512
+    unsigned slab_stride;                     // elements between tiles adjacent in z  = TX*TY*512
+    float vmin, inv_range;                    // O6
+    float ert;                                // O7 threshold
+    int ert_on;
+};
+
+struct BrickRec {
+    int lo[3], hi[3];         // brick box (voxels)
+    int rx0, ry0, rw, rh;     // rendering rectangle (pixels)
+    int tile0, tiles_x;       // first CTA index of this brick, CTAs per rectangle row
+    long long img_base;       // pixel offset of this brick's image in the image buffer
+    int img_stride, ox, oy;   // row stride (pixels) and pixel coordinates of image element (0,0)
+    int pad;
+};
+
+// ------------------------------------------------------------------------------------------------
+// a0  re-layout.  One CTA moves an 8(z) x 8(y) x 64(x) block: coalesced row reads -> shared memory
+// -> 8 whole tiles written as one contiguous 16 KB run of float4 stores.  Source indices are
+// clamped, so the padding voxels replicate the cube's faces (this makes
+// x+1 / y+1 / z+1 of any in-range voxel addressable without a bounds test, with the same result as
+// the clamp of O5 because the weight of the replicated voxel is then exactly zero).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+relayout_kernel(const float* __restrict__ src, float* __restrict__ dst, int nx, int ny, int nz,
+                int TX, int TY) {
+    __shared__ __align__(16) float sm[64][72];   // row = lz*8+ly; 72-float pitch: conflict-free float4 reads
+    const int tx0 = blockIdx.x * 8, ty = blockIdx.y, tz = blockIdx.z;
+    const int t = threadIdx.x;
+    const int xo = t & 63;
+    const int xs = min(tx0 * 8 + xo, nx - 1);
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+        const int row = (t >> 6) + 4 * k;
+        const int z = min(tz * 8 + (row >> 3), nz - 1);
+        const int y = min(ty * 8 + (row & 7), ny - 1);
+        sm[row][xo] = __ldcs(src + ((size_t)z * ny + y) * nx + xs);
+    }
+    __syncthreads();
+    const int ntile = min(8, TX - tx0);
+    float4* out = reinterpret_cast<float4*>(dst + ((size_t)((size_t)tz * TY + ty) * TX + tx0) * TILE_ELEMS);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int j = t + 256 * k;           // float4 index inside the 8-tile run
+        const int tile = j >> 7, r = j & 127;
+        if (tile < ntile) {
+            const int row = r >> 1, lxq = r & 1;
+            const float4 v = *reinterpret_cast<const float4*>(&sm[row][tile * 8 + lxq * 4]);
+            out[j] = v;
+        }
+    }
+}
+
+// element offset of voxel (x,y,z) in the tiled copy
+__device__ __forceinline__ size_t tiled_index(int x, int y, int z, unsigned ty_stride, unsigned slab_stride) {
+    return (size_t)(z >> 3) * slab_stride + (size_t)(y >> 3) * ty_stride + (size_t)(x >> 3) * TILE_ELEMS +
+           (size_t)(((z & 7) << 6) | ((y & 7) << 3) | (x & 7));
+}
+
+// inverse of a0 (round-trip test only)
+__global__ void export_linear_kernel(const float* __restrict__ tiled, float* __restrict__ dst, int nx, int ny,
+                                     int nz, unsigned ty_stride, unsigned slab_stride) {
+    const size_t n = (size_t)nx * ny * nz;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const int x = (int)(i % nx);
+        const size_t r = i / nx;
+        const int y = (int)(r % ny), z = (int)(r / ny);
+        dst[i] = tiled[tiled_index(x, y, z, ty_stride, slab_stride)];
+    }
+}
+
+__global__ void fill_kernel(float* __restrict__ p, size_t n, float v) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+        p[i] = v;
+}
+
+// ------------------------------------------------------------------------------------------------
+// per-ray set-up in double (O2, O3, O4, O9)
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void make_ray(const FrameParams& P, int px, int py, double o[3], double d[3]) {
+    const double u = 2.0 * ((double)px + 0.5) / (double)P.W - 1.0;
+    const double v = 2.0 * ((double)py + 0.5) / (double)P.H - 1.0;
+    if (P.proj == 0) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            o[c] = P.eye[c] + u * P.h * P.asp * P.right[c] + v * P.h * P.up[c];
+            d[c] = P.fwd[c];
+        }
+    } else {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            o[c] = P.eye[c];
+            d[c] = P.fwd[c] + u * P.tanhalf * P.asp * P.right[c] + v * P.tanhalf * P.up[c];
+        }
+        const double l = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+        d[0] /= l; d[1] /= l; d[2] /= l;
+    }
+}
+
+// O3 slab clip against [lo,hi]; t0 is not clamped to >= 0 here.
+__device__ __forceinline__ bool slab_clip(const double o[3], const double d[3], const double lo[3],
+                                          const double hi[3], double& tn, double& tf) {
+    tn = -INFINITY; tf = INFINITY;
+    bool ok = true;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        if (d[a] == 0.0) {
+            if (!(lo[a] <= o[a] && o[a] < hi[a])) ok = false;
+        } else {
+            const double t0 = (lo[a] - o[a]) / d[a];
+            const double t1 = (hi[a] - o[a]) / d[a];
+            const double tmin = t0 < t1 ? t0 : t1;
+            const double tmax = t0 < t1 ? t1 : t0;
+            if (tmin > tn) tn = tmin;
+            if (tmax < tf) tf = tmax;
+        }
+    }
+    return ok;
+}
+
+// O4: I(t) = max(0, ceil((t - t_near)/step - 1/2))
+__device__ __forceinline__ long long lattice_index(double t, double t_near, double step) {
+    const double x = ceil((t - t_near) / step - 0.5);
+    return x > 0.0 ? (long long)x : 0ll;
+}
+
+// ------------------------------------------------------------------------------------------------
+// O5  trilinear sample of the tiled cube at (qx,qy,qz) = position - 1/2, fp32.
+// ------------------------------------------------------------------------------------------------
+struct Footprint {           // the 8 voxels of one sample and its fractional weights
+    float v[8];
+    float fx, fy, fz;
+};
+
+template <int INSTR>
+__device__ __forceinline__ void fetch(const float* __restrict__ vol, const FrameParams& P, float nxm1, float nym1,
+                                      float nzm1, float qx, float qy, float qz, Footprint& F,
+                                      unsigned* __restrict__ bitmap) {
+    qx = fminf(fmaxf(qx, 0.0f), nxm1);
+    qy = fminf(fmaxf(qy, 0.0f), nym1);
+    qz = fminf(fmaxf(qz, 0.0f), nzm1);
+    // floor of a non-negative float < 2^22 without F2I/I2F: add 2^23 rounding down, the integer is
+    // then the low mantissa bits and (r - 2^23) is that integer as a float, exactly.
+    const float rx = __fadd_rd(qx, 8388608.0f), ry = __fadd_rd(qy, 8388608.0f), rz = __fadd_rd(qz, 8388608.0f);
+    const unsigned ix = __float_as_uint(rx) & 0x7fffffu, iy = __float_as_uint(ry) & 0x7fffffu,
+                   iz = __float_as_uint(rz) & 0x7fffffu;
+    F.fx = qx - (rx - 8388608.0f);
+    F.fy = qy - (ry - 8388608.0f);
+    F.fz = qz - (rz - 8388608.0f);
+    // separable tiled offsets; +1 neighbours always exist (padding), see relayout_kernel
+    const unsigned ix1 = ix + 1, iy1 = iy + 1, iz1 = iz + 1;
+    const unsigned ex0 = (ix >> 3) * TILE_ELEMS + (ix & 7), ex1 = (ix1 >> 3) * TILE_ELEMS + (ix1 & 7);
+    const unsigned ey0 = (iy >> 3) * P.ty_stride + ((iy & 7) << 3), ey1 = (iy1 >> 3) * P.ty_stride + ((iy1 & 7) << 3);
+    const float* __restrict__ pz0 = vol + (size_t)(iz >> 3) * P.slab_stride + ((iz & 7) << 6);
+    const float* __restrict__ pz1 = vol + (size_t)(iz1 >> 3) * P.slab_stride + ((iz1 & 7) << 6);
+    const unsigned e00 = ex0 + ey0, e10 = ex1 + ey0, e01 = ex0 + ey1, e11 = ex1 + ey1;
+    F.v[0] = __ldg(pz0 + e00); F.v[1] = __ldg(pz0 + e10);
+    F.v[2] = __ldg(pz0 + e01); F.v[3] = __ldg(pz0 + e11);
+    F.v[4] = __ldg(pz1 + e00); F.v[5] = __ldg(pz1 + e10);
+    F.v[6] = __ldg(pz1 + e01); F.v[7] = __ldg(pz1 + e11);
+    if (INSTR) {   // mark the 32-byte sectors (8 consecutive floats) of the footprint
+        const size_t b0 = (size_t)(pz0 - vol), b1 = (size_t)(pz1 - vol);
+        const size_t s[8] = {(b0 + e00) >> 3, (b0 + e10) >> 3, (b0 + e01) >> 3, (b0 + e11) >> 3,
+                             (b1 + e00) >> 3, (b1 + e10) >> 3, (b1 + e01) >> 3, (b1 + e11) >> 3};
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const unsigned bit = 1u << (unsigned)(s[k] & 31);
+            unsigned* w = bitmap + (s[k] >> 5);
+            if (!(*(volatile unsigned*)w & bit)) atomicOr(w, bit);
+        }
+    }
+}
+
+__device__ __forceinline__ float trilerp(const Footprint& F) {
+    const float c00 = fmaf(F.fx, F.v[1] - F.v[0], F.v[0]);
+    const float c10 = fmaf(F.fx, F.v[3] - F.v[2], F.v[2]);
+    const float c01 = fmaf(F.fx, F.v[5] - F.v[4], F.v[4]);
+    const float c11 = fmaf(F.fx, F.v[7] - F.v[6], F.v[6]);
+    const float c0 = fmaf(F.fy, c10 - c00, c00);
+    const float c1 = fmaf(F.fy, c11 - c01, c01);
+    return fmaf(F.fz, c1 - c0, c0);
+}
+
+// O6 + O7: classify through the shared-memory table (entry m: T[m], then T[m+1]-T[m]) and blend.
+__device__ __forceinline__ void classify_blend(const float4* __restrict__ tf, const FrameParams& P, float value,
+                                               float& Cr, float& Cg, float& Cb, float& A) {
+    const float x = __saturatef((value - P.vmin) * P.inv_range) * 255.0f;
+    const float r = fminf(__fadd_rd(x, 8388608.0f), 8388608.0f + 254.0f);   // 2^23 + min(floor(x),254)
+    const unsigned m = __float_as_uint(r) & 0xffu;
+    const float w = x - (r - 8388608.0f);
+    const float4 t0 = tf[2 * m], dt = tf[2 * m + 1];
+    float a = fmaf(w, dt.w, t0.w);
+    a = (value == value) ? a : 0.0f;                                         // O5/A14: NaN sample skipped
+    const float wgt = (1.0f - A) * a;
+    Cr = fmaf(wgt, fmaf(w, dt.x, t0.x), Cr);
+    Cg = fmaf(wgt, fmaf(w, dt.y, t0.y), Cg);
+    Cb = fmaf(wgt, fmaf(w, dt.z, t0.z), Cb);
+    A += wgt;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1 + a3 + a4/a5  the caster.  grid.x = sum over bricks of the 16x16-pixel tiles of their
+// rendering rectangles; block = 256 threads = 8 warps, each an 8x4-pixel patch.
+// INSTR = 1 is the measuring build (samples evaluated, sector bitmap), never the product path.
+// ------------------------------------------------------------------------------------------------
+template <int MODE, int INSTR>
+__global__ void __launch_bounds__(CTA_THREADS)
+cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ bricks, int n_bricks,
+            const float* __restrict__ vol, const float4* __restrict__ tf_global, float* __restrict__ img,
+            unsigned long long* __restrict__ counters, unsigned* __restrict__ bitmap) {
+    __shared__ __align__(16) float4 tf[MODE == MODE_EA ? 512 : 1];
+    __shared__ int s_brick;
+    if (MODE == MODE_EA) {
+        tf[threadIdx.x] = tf_global[threadIdx.x];
+        tf[threadIdx.x + 256] = tf_global[threadIdx.x + 256];
+    }
+    if (threadIdx.x == 0) {               // which brick owns this CTA: last brick with tile0 <= blockIdx.x
+        int lo = 0, hi = n_bricks - 1;
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (bricks[mid].tile0 <= (int)blockIdx.x) lo = mid; else hi = mid - 1;
+        }
+        s_brick = lo;
+    }
+    __syncthreads();
+    const BrickRec* __restrict__ br = bricks + s_brick;
+    const int tloc = (int)blockIdx.x - br->tile0;
+    const int tiles_x = br->tiles_x;
+    const int tyi = tloc / tiles_x, txi = tloc - tyi * tiles_x;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int lx = txi * CTA_PX + (warp & 1) * 8 + (lane & 7);
+    const int ly = tyi * CTA_PX + (warp >> 1) * 4 + (lane >> 3);
+    if (lx >= br->rw || ly >= br->rh) return;
+    const int px = br->rx0 + lx, py = br->ry0 + ly;
+
+    // ---- per-ray set-up, double precision (O2-O4, O9) ----
+    double o[3], d[3];
+    make_ray(P, px, py, o, d);
+    long long i_lo = 0, i_hi = 0;
+    double t_near = 0.0;
+    {
+        const double glo[3] = {0.0, 0.0, 0.0};
+        const double ghi[3] = {(double)P.nx, (double)P.ny, (double)P.nz};
+        double tn, tf_;
+        bool hit = slab_clip(o, d, glo, ghi, tn, tf_);
+        if (tn < 0.0) tn = 0.0;
+        hit = hit && (tf_ > tn);
+        if (hit) {
+            t_near = tn;
+            const double blo[3] = {(double)br->lo[0], (double)br->lo[1], (double)br->lo[2]};
+            const double bhi[3] = {(double)br->hi[0], (double)br->hi[1], (double)br->hi[2]};
+            double t0, t1;
+            bool bh = slab_clip(o, d, blo, bhi, t0, t1);
+            if (t0 < tn) t0 = tn;
+            if (t1 > tf_) t1 = tf_;
+            if (bh && t1 > t0) {
+                i_lo = lattice_index(t0, tn, P.step);
+                i_hi = lattice_index(t1, tn, P.step);
+            }
+        }
+    }
+    const int n = (i_hi > i_lo) ? (int)(i_hi - i_lo) : 0;
+
+    const size_t pix = (size_t)br->img_base + (size_t)(py - br->oy) * br->img_stride + (size_t)(px - br->ox);
+    if (n == 0) {
+        if (MODE == MODE_EA) reinterpret_cast<float4*>(img)[pix] = make_float4(0.f, 0.f, 0.f, 0.f);
+        else img[pix] = -INFINITY;
+        return;
+    }
+    // anchor the brick's first sample in double, then march in fp32: q_j = q0 + j*ds  (q = position - 1/2)
+    const double ta = t_near + ((double)i_lo + 0.5) * P.step;
+    const float q0x = (float)(o[0] + ta * d[0] - 0.5), q0y = (float)(o[1] + ta * d[1] - 0.5),
+                q0z = (float)(o[2] + ta * d[2] - 0.5);
+    const double dsx = P.step * d[0], dsy = P.step * d[1], dsz = P.step * d[2];
+    const float hx = (float)dsx, hy = (float)dsy, hz = (float)dsz;                 // step vector, high part
+    const float ex = (float)(dsx - (double)hx), ey = (float)(dsy - (double)hy), ez = (float)(dsz - (double)hz);
+    const float nxm1 = (float)(P.nx - 1), nym1 = (float)(P.ny - 1), nzm1 = (float)(P.nz - 1);
+
+    float Cr = 0.f, Cg = 0.f, Cb = 0.f, A = 0.f, M = -INFINITY;
+    unsigned long long count = 0;
+    if (INSTR) {
+        for (int j = 0; j < n; ++j) {
+            const float jf = (float)j;
+            Footprint F;
+            fetch<1>(vol, P, nxm1, nym1, nzm1, fmaf(jf, hx, fmaf(jf, ex, q0x)), fmaf(jf, hy, fmaf(jf, ey, q0y)),
+                     fmaf(jf, hz, fmaf(jf, ez, q0z)), F, bitmap);
+            const float v = trilerp(F);
+            ++count;
+            if (MODE == MODE_EA) {
+                classify_blend(tf, P, v, Cr, Cg, Cb, A);
+                if (P.ert_on && A >= P.ert) break;
+            } else {
+                M = fmaxf(M, v);
+            }
+        }
+        if (counters) atomicAdd(counters, count);
+    } else {
+        // two samples in flight per iteration: 16 independent loads before the first blend
+        for (int j = 0; j < n; j += 2) {
+            const float j0 = (float)j, j1 = (float)(j + 1);
+            Footprint F0, F1;
+            fetch<0>(vol, P, nxm1, nym1, nzm1, fmaf(j0, hx, fmaf(j0, ex, q0x)), fmaf(j0, hy, fmaf(j0, ey, q0y)),
+                     fmaf(j0, hz, fmaf(j0, ez, q0z)), F0, nullptr);
+            fetch<0>(vol, P, nxm1, nym1, nzm1, fmaf(j1, hx, fmaf(j1, ex, q0x)), fmaf(j1, hy, fmaf(j1, ey, q0y)),
+                     fmaf(j1, hz, fmaf(j1, ez, q0z)), F1, nullptr);
+            const float v0 = trilerp(F0), v1 = trilerp(F1);
+            if (MODE == MODE_EA) {
+                classify_blend(tf, P, v0, Cr, Cg, Cb, A);
+                if (P.ert_on && A >= P.ert) break;
+                if (j + 1 < n) {
+                    classify_blend(tf, P, v1, Cr, Cg, Cb, A);
+                    if (P.ert_on && A >= P.ert) break;
+                }
+            } else {
+                M = fmaxf(M, v0);
+                if (j + 1 < n) M = fmaxf(M, v1);
+            }
+        }
+    }
+    if (MODE == MODE_EA) reinterpret_cast<float4*>(img)[pix] = make_float4(Cr, Cg, Cb, A);
+    else img[pix] = M;
+}
+
+// number of set bits of the sector bitmap (measuring build only)
+__global__ void popcount_kernel(const unsigned* __restrict__ bitmap, size_t n_words, unsigned long long* out) {
+    unsigned long long c = 0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_words; i += (size_t)gridDim.x * blockDim.x)
+        c += __popc(bitmap[i]);
+    for (int s = 16; s > 0; s >>= 1) c += __shfl_xor_sync(0xffffffffu, c, s);
+    if ((threadIdx.x & 31) == 0 && c) atomicAdd(out, c);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a7  sort-last composite.  One thread per pixel walks the bricks front to back
+// (order[] from the host, A11) and applies "over" (EA) or max (MIP, then the O8 colour lookup in the
+// uncorrected table).  A brick is skipped by the whole warp when none of its 32 pixels lies inside
+// the brick's rendering rectangle (warp vote), so the cost per pixel is the depth complexity, not B.
+// ------------------------------------------------------------------------------------------------
+template <int MODE>
+__global__ void __launch_bounds__(256)
+composite_kernel(const BrickRec* __restrict__ bricks, const int* __restrict__ order, int n_bricks,
+                 const float* __restrict__ img, int W, int H, const float4* __restrict__ tf_raw, float vmin,
+                 float inv_range, float* __restrict__ out_rgba, float* __restrict__ out_scalar) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int px = blockIdx.x * 16 + (warp & 1) * 8 + (lane & 7);
+    const int py = blockIdx.y * 16 + (warp >> 1) * 4 + (lane >> 3);
+    const bool live = px < W && py < H;
+    float Cr = 0.f, Cg = 0.f, Cb = 0.f, Tr = 1.f, M = -INFINITY;
+    for (int k = 0; k < n_bricks; ++k) {
+        const BrickRec* __restrict__ br = bricks + order[k];
+        const bool in = live && px >= br->rx0 && px < br->rx0 + br->rw && py >= br->ry0 && py < br->ry0 + br->rh;
+        if (!__any_sync(0xffffffffu, in)) continue;
+        if (in) {
+            const size_t pix = (size_t)br->img_base + (size_t)(py - br->oy) * br->img_stride + (size_t)(px - br->ox);
+            if (MODE == MODE_EA) {
+                const float4 v = __ldcs(reinterpret_cast<const float4*>(img) + pix);
+                Cr = fmaf(Tr, v.x, Cr); Cg = fmaf(Tr, v.y, Cg); Cb = fmaf(Tr, v.z, Cb);
+                Tr *= (1.0f - v.w);
+            } else {
+                M = fmaxf(M, __ldcs(img + pix));
+            }
+        }
+    }
+    if (!live) return;
+    const size_t o = (size_t)py * W + px;
+    if (MODE == MODE_EA) {
+        reinterpret_cast<float4*>(out_rgba)[o] = make_float4(Cr, Cg, Cb, 1.0f - Tr);
+    } else {
+        if (out_scalar) out_scalar[o] = M;
+        float4 e = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (M != -INFINITY) {       // O8: colour of the maximum, uncorrected table, un-premultiplied
+            const float x = __saturatef((M - vmin) * inv_range) * 255.0f;
+            const int m = min((int)x, 254);
+            const float w = x - (float)m;
+            const float4 t0 = tf_raw[m], t1 = tf_raw[m + 1];
+            e = make_float4(fmaf(w, t1.x - t0.x, t0.x), fmaf(w, t1.y - t0.y, t0.y), fmaf(w, t1.z - t0.z, t0.z),
+                            fmaf(w, t1.w - t0.w, t0.w));
+        }
+        reinterpret_cast<float4*>(out_rgba)[o] = e;
+    }
+}
+
+}  // namespace vr

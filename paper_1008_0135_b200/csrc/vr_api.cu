@@ -1,0 +1,439 @@
+// vr_api.cu — the C ABI of include/vr.h: argument checks, per-frame planning on the host (plan.h)
+// and kernel launches (kernels.cuh).  Every step of the path runs in the kernels; this file only
+// validates, plans and enqueues.  There is no CPU fallback.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/vr.h"
+#include "kernels.cuh"
+#include "plan.h"
+
+namespace {
+
+thread_local std::string g_err;
+
+vr_status fail(vr_status s, const std::string& msg) {
+    g_err = msg;
+    return s;
+}
+vr_status cuda_fail(cudaError_t e, const char* what) {
+    vr_status s = (e == cudaErrorMemoryAllocation) ? VR_ERR_OOM : VR_ERR_CUDA;
+    return fail(s, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define VR_CUDA(call, what)                                   \
+    do {                                                      \
+        cudaError_t e_ = (call);                              \
+        if (e_ != cudaSuccess) return cuda_fail(e_, what);    \
+    } while (0)
+
+}  // namespace
+
+struct vr_volume {
+    int dims[3] = {0, 0, 0};
+    int TX = 0, TY = 0, TZ = 0;
+    size_t tiled_elems = 0;
+    float* d_tiled = nullptr;
+    cudaStream_t stream = nullptr;
+    float relayout_ms = 0.f;
+
+    bool has_tf = false;
+    float tf_host[1024];
+    float vmin = 0.f, vmax = 1.f;
+    double tf_step = -1.0;            // step the device EA table is currently corrected for
+    float4* d_tf_ea = nullptr;        // 512 float4: T_step[m], T_step[m+1]-T_step[m]
+    float4* d_tf_raw = nullptr;       // 256 float4: table as given (MIP colour, O8)
+
+    int bricks[3] = {1, 1, 1};
+    vr::BrickRec* d_bricks = nullptr; // VR_MAX_BRICKS records
+    int* d_order = nullptr;
+
+    float* d_pool = nullptr;          // rect-cropped brick images of vr_render
+    size_t pool_floats = 0;
+    float* d_frame = nullptr;         // internal frame of vr_render_to_host
+    size_t frame_floats = 0;
+};
+
+namespace {
+
+struct Frame {                         // everything one frame needs, built on the host
+    vr::FrameParams P;
+    std::vector<vr::BrickRec> recs;
+    std::vector<int> order;
+    int total_tiles = 0;
+    size_t pool_pixels = 0;
+};
+
+vr_status check_render_args(const vr_volume* vol, const vr_camera* cam, int W, int H, float step, int mode) {
+    if (!vol) return fail(VR_ERR_INVALID_ARG, "volume is NULL");
+    if (!cam) return fail(VR_ERR_INVALID_ARG, "camera is NULL");
+    if (W <= 0 || H <= 0 || W > 32768 || H > 32768) return fail(VR_ERR_INVALID_ARG, "W and H must be in [1,32768]");
+    if (!(step > 0.0f) || !std::isfinite(step)) return fail(VR_ERR_INVALID_ARG, "step_voxels must be positive and finite");
+    if (mode != VR_MODE_EA && mode != VR_MODE_MIP) return fail(VR_ERR_INVALID_ARG, "unknown mode");
+    if (const char* why = vr::check_camera(*cam)) return fail(VR_ERR_INVALID_ARG, why);
+    const double diag = std::sqrt((double)vol->dims[0] * vol->dims[0] + (double)vol->dims[1] * vol->dims[1] +
+                                  (double)vol->dims[2] * vol->dims[2]);
+    if (diag / (double)step > 8.0e6) return fail(VR_ERR_INVALID_ARG, "step_voxels too small for this volume (> 8e6 samples per ray)");
+    if (!vol->has_tf) return fail(VR_ERR_STATE, "no transfer function set (vr_set_transfer_function)");
+    return VR_OK;
+}
+
+// cropped = true: brick images are rect-sized and packed (vr_render); false: full W x H frames.
+void build_frame(const vr_volume* vol, const vr_camera* cam, int W, int H, float step, float ert, bool cropped,
+                 bool direct, Frame& f) {
+    const vr::Basis bs = vr::make_basis(*cam);
+    vr::FrameParams& P = f.P;
+    for (int c = 0; c < 3; ++c) {
+        P.eye[c] = bs.eye[c]; P.right[c] = bs.right[c]; P.up[c] = bs.up[c]; P.fwd[c] = bs.fwd[c];
+    }
+    P.h = (double)cam->ortho_half_h;
+    P.asp = (double)W / (double)H;
+    P.tanhalf = cam->projection == VR_PROJ_PERSP ? vr::tan_half_fov(*cam) : 0.0;
+    P.step = (double)step;
+    P.proj = cam->projection; P.W = W; P.H = H;
+    P.nx = vol->dims[0]; P.ny = vol->dims[1]; P.nz = vol->dims[2];
+    P.ty_stride = (unsigned)vol->TX * vr::TILE_ELEMS;
+    P.slab_stride = (unsigned)vol->TX * (unsigned)vol->TY * vr::TILE_ELEMS;
+    P.vmin = vol->vmin;
+    P.inv_range = 1.0f / (vol->vmax - vol->vmin);
+    P.ert_on = (ert > 0.0f && ert < 1.0f) ? 1 : 0;
+    P.ert = ert;
+
+    std::vector<vr::BrickPlan> plan;
+    vr::plan_bricks(vol->dims, vol->bricks, *cam, W, H, plan, f.order);
+    const int B = (int)plan.size();
+    f.recs.assign(B, vr::BrickRec());
+    int tiles = 0;
+    size_t pool = 0;
+    // CTAs are laid out brick by brick, front to back
+    for (int k = 0; k < B; ++k) {
+        const int b = f.order[k];
+        vr::BrickPlan bp = plan[b];
+        if (direct) { bp.rx0 = 0; bp.ry0 = 0; bp.rw = W; bp.rh = H; }   // one brick writes the frame itself
+        vr::BrickRec& r = f.recs[b];
+        for (int a = 0; a < 3; ++a) { r.lo[a] = bp.lo[a]; r.hi[a] = bp.hi[a]; }
+        r.rx0 = bp.rx0; r.ry0 = bp.ry0; r.rw = bp.rw; r.rh = bp.rh;
+        r.tile0 = tiles;
+        r.tiles_x = (bp.rw + vr::CTA_PX - 1) / vr::CTA_PX;
+        const int tiles_y = (bp.rh + vr::CTA_PX - 1) / vr::CTA_PX;
+        tiles += r.tiles_x * tiles_y;
+        if (cropped && !direct) {
+            r.img_base = (long long)pool; r.img_stride = bp.rw; r.ox = bp.rx0; r.oy = bp.ry0;
+            pool += (size_t)bp.rw * bp.rh;
+        } else {
+            r.img_base = direct ? 0 : (long long)b * W * H; r.img_stride = W; r.ox = 0; r.oy = 0;
+        }
+        r.pad = 0;
+    }
+    f.total_tiles = tiles;
+    f.pool_pixels = pool;
+}
+
+// The cast kernel looks its brick up by tile0 with a binary search over records in FRONT-TO-BACK order;
+// recs[] is indexed by brick id, so upload a copy sorted by order[] for the caster and keep ids for
+// the compositor: simplest is to store records in order[] sequence and make order[] the identity.
+vr_status upload_plan(vr_volume* vol, Frame& f) {
+    const int B = (int)f.recs.size();
+    std::vector<vr::BrickRec> sorted(B);
+    std::vector<int> ident(B);
+    for (int k = 0; k < B; ++k) { sorted[k] = f.recs[f.order[k]]; ident[k] = k; }
+    VR_CUDA(cudaMemcpyAsync(vol->d_bricks, sorted.data(), sizeof(vr::BrickRec) * B, cudaMemcpyHostToDevice, vol->stream),
+            "upload brick table");
+    VR_CUDA(cudaMemcpyAsync(vol->d_order, ident.data(), sizeof(int) * B, cudaMemcpyHostToDevice, vol->stream),
+            "upload brick order");
+    return VR_OK;
+}
+
+// O6: per-entry opacity correction for this step, in double, then the (T, dT) pairs the caster reads.
+vr_status upload_tf_for_step(vr_volume* vol, double step) {
+    if (vol->tf_step == step) return VR_OK;
+    std::vector<float> t(256 * 4);
+    for (int j = 0; j < 256; ++j) {
+        for (int c = 0; c < 3; ++c) t[4 * j + c] = vol->tf_host[4 * j + c];
+        const double a = (double)vol->tf_host[4 * j + 3];
+        t[4 * j + 3] = (float)((step == 1.0) ? a : 1.0 - std::pow(1.0 - a, step));
+    }
+    std::vector<float> pairs(512 * 4, 0.0f);
+    for (int m = 0; m < 256; ++m)
+        for (int c = 0; c < 4; ++c) {
+            pairs[8 * m + c] = t[4 * m + c];
+            pairs[8 * m + 4 + c] = (m < 255) ? (float)((double)t[4 * (m + 1) + c] - (double)t[4 * m + c]) : 0.0f;
+        }
+    VR_CUDA(cudaMemcpyAsync(vol->d_tf_ea, pairs.data(), sizeof(float) * 2048, cudaMemcpyHostToDevice, vol->stream),
+            "upload transfer function");
+    vol->tf_step = step;
+    return VR_OK;
+}
+
+template <int INSTR>
+vr_status launch_cast(vr_volume* vol, const Frame& f, int mode, float* d_img, unsigned long long* d_counter,
+                      unsigned* d_bitmap) {
+    if (f.total_tiles == 0) return VR_OK;
+    const int B = (int)f.recs.size();
+    if (mode == VR_MODE_EA)
+        vr::cast_kernel<vr::MODE_EA, INSTR><<<f.total_tiles, vr::CTA_THREADS, 0, vol->stream>>>(
+            f.P, vol->d_bricks, B, vol->d_tiled, vol->d_tf_ea, d_img, d_counter, d_bitmap);
+    else
+        vr::cast_kernel<vr::MODE_MIP, INSTR><<<f.total_tiles, vr::CTA_THREADS, 0, vol->stream>>>(
+            f.P, vol->d_bricks, B, vol->d_tiled, vol->d_tf_ea, d_img, d_counter, d_bitmap);
+    VR_CUDA(cudaGetLastError(), "cast kernel launch");
+    return VR_OK;
+}
+
+vr_status launch_composite(vr_volume* vol, const Frame& f, int mode, const float* d_img, int W, int H, float* d_out,
+                           float* d_scalar) {
+    const int B = (int)f.recs.size();
+    dim3 grid((W + 15) / 16, (H + 15) / 16);
+    if (mode == VR_MODE_EA)
+        vr::composite_kernel<vr::MODE_EA><<<grid, 256, 0, vol->stream>>>(vol->d_bricks, vol->d_order, B, d_img, W, H,
+                                                                         vol->d_tf_raw, f.P.vmin, f.P.inv_range, d_out, d_scalar);
+    else
+        vr::composite_kernel<vr::MODE_MIP><<<grid, 256, 0, vol->stream>>>(vol->d_bricks, vol->d_order, B, d_img, W, H,
+                                                                          vol->d_tf_raw, f.P.vmin, f.P.inv_range, d_out, d_scalar);
+    VR_CUDA(cudaGetLastError(), "composite kernel launch");
+    return VR_OK;
+}
+
+vr_status ensure_pool(vr_volume* vol, size_t floats) {
+    if (floats <= vol->pool_floats) return VR_OK;
+    if (vol->d_pool) { cudaFree(vol->d_pool); vol->d_pool = nullptr; vol->pool_floats = 0; }
+    const size_t want = floats + floats / 4;
+    VR_CUDA(cudaMalloc(&vol->d_pool, want * sizeof(float)), "allocate brick images");
+    vol->pool_floats = want;
+    return VR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* vr_last_error(void) { return g_err.c_str(); }
+
+vr_status vr_create_volume(const int dims[3], const float* d_data, vr_volume** out) {
+    if (!dims || !d_data || !out) return fail(VR_ERR_INVALID_ARG, "vr_create_volume: NULL argument");
+    *out = nullptr;
+    for (int a = 0; a < 3; ++a)
+        if (dims[a] <= 0 || dims[a] > 65528) return fail(VR_ERR_INVALID_ARG, "vr_create_volume: each dim must be in [1,65528]");
+    vr_volume* v = new (std::nothrow) vr_volume();
+    if (!v) return fail(VR_ERR_OOM, "vr_create_volume: host allocation failed");
+    for (int a = 0; a < 3; ++a) v->dims[a] = dims[a];
+    v->TX = (dims[0] + 1 + 7) / 8; v->TY = (dims[1] + 1 + 7) / 8; v->TZ = (dims[2] + 1 + 7) / 8;
+    if ((double)v->TX * v->TY * vr::TILE_ELEMS >= 4294967296.0) {
+        delete v;
+        return fail(VR_ERR_INVALID_ARG, "vr_create_volume: nx*ny too large for 32-bit in-slab offsets");
+    }
+    v->tiled_elems = (size_t)v->TX * v->TY * v->TZ * vr::TILE_ELEMS;
+    cudaError_t e = cudaMalloc(&v->d_tiled, v->tiled_elems * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc(&v->d_tf_ea, 512 * sizeof(float4));
+    if (e == cudaSuccess) e = cudaMalloc(&v->d_tf_raw, 256 * sizeof(float4));
+    if (e == cudaSuccess) e = cudaMalloc(&v->d_bricks, VR_MAX_BRICKS * sizeof(vr::BrickRec));
+    if (e == cudaSuccess) e = cudaMalloc(&v->d_order, VR_MAX_BRICKS * sizeof(int));
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (e == cudaSuccess) e = cudaEventCreate(&e0);
+    if (e == cudaSuccess) e = cudaEventCreate(&e1);
+    if (e == cudaSuccess) {
+        dim3 grid((v->TX + 7) / 8, v->TY, v->TZ);
+        cudaEventRecord(e0, v->stream);
+        vr::relayout_kernel<<<grid, 256, 0, v->stream>>>(d_data, v->d_tiled, dims[0], dims[1], dims[2], v->TX, v->TY);
+        cudaEventRecord(e1, v->stream);
+        e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaStreamSynchronize(v->stream);
+        if (e == cudaSuccess) cudaEventElapsedTime(&v->relayout_ms, e0, e1);
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (e != cudaSuccess) {
+        vr_status s = cuda_fail(e, "vr_create_volume");
+        vr_destroy_volume(v);
+        return s;
+    }
+    *out = v;
+    return VR_OK;
+}
+
+void vr_destroy_volume(vr_volume* v) {
+    if (!v) return;
+    if (v->d_tiled) cudaFree(v->d_tiled);
+    if (v->d_tf_ea) cudaFree(v->d_tf_ea);
+    if (v->d_tf_raw) cudaFree(v->d_tf_raw);
+    if (v->d_bricks) cudaFree(v->d_bricks);
+    if (v->d_order) cudaFree(v->d_order);
+    if (v->d_pool) cudaFree(v->d_pool);
+    if (v->d_frame) cudaFree(v->d_frame);
+    delete v;
+}
+
+vr_status vr_set_stream(vr_volume* vol, void* cuda_stream) {
+    if (!vol) return fail(VR_ERR_INVALID_ARG, "vr_set_stream: volume is NULL");
+    vol->stream = (cudaStream_t)cuda_stream;
+    return VR_OK;
+}
+
+vr_status vr_set_transfer_function(vr_volume* vol, const float rgba[1024], float vmin, float vmax) {
+    if (!vol || !rgba) return fail(VR_ERR_INVALID_ARG, "vr_set_transfer_function: NULL argument");
+    if (!std::isfinite(vmin) || !std::isfinite(vmax) || !(vmax > vmin))
+        return fail(VR_ERR_INVALID_ARG, "vr_set_transfer_function: need finite vmin < vmax");
+    for (int i = 0; i < 1024; ++i)
+        if (!(rgba[i] >= 0.0f && rgba[i] <= 1.0f))
+            return fail(VR_ERR_INVALID_ARG, "vr_set_transfer_function: table entries must be in [0,1]");
+    std::memcpy(vol->tf_host, rgba, sizeof(float) * 1024);
+    vol->vmin = vmin; vol->vmax = vmax;
+    vol->tf_step = -1.0;
+    VR_CUDA(cudaMemcpyAsync(vol->d_tf_raw, vol->tf_host, sizeof(float) * 1024, cudaMemcpyHostToDevice, vol->stream),
+            "upload transfer function");
+    vol->has_tf = true;
+    return VR_OK;
+}
+
+vr_status vr_set_bricks(vr_volume* vol, int bx, int by, int bz) {
+    if (!vol) return fail(VR_ERR_INVALID_ARG, "vr_set_bricks: volume is NULL");
+    const int b[3] = {bx, by, bz};
+    for (int a = 0; a < 3; ++a)
+        if (b[a] < 1 || b[a] > vol->dims[a]) return fail(VR_ERR_INVALID_ARG, "vr_set_bricks: need 1 <= b_a <= n_a");
+    if ((long long)bx * by * bz > VR_MAX_BRICKS) return fail(VR_ERR_INVALID_ARG, "vr_set_bricks: more than VR_MAX_BRICKS bricks");
+    for (int a = 0; a < 3; ++a) vol->bricks[a] = b[a];
+    return VR_OK;
+}
+
+vr_status vr_render(vr_volume* vol, const vr_camera* cam, int W, int H, float step, int mode, float ert,
+                    float* d_out_rgba, float* d_out_scalar) {
+    vr_status s = check_render_args(vol, cam, W, H, step, mode);
+    if (s != VR_OK) return s;
+    if (!d_out_rgba) return fail(VR_ERR_INVALID_ARG, "vr_render: d_out_rgba is NULL");
+    const int B = vol->bricks[0] * vol->bricks[1] * vol->bricks[2];
+    const bool direct = (B == 1 && mode == VR_MODE_EA);
+    Frame f;
+    build_frame(vol, cam, W, H, step, ert, true, direct, f);
+    if ((s = upload_plan(vol, f)) != VR_OK) return s;
+    if (mode == VR_MODE_EA && (s = upload_tf_for_step(vol, (double)step)) != VR_OK) return s;
+    if (direct) return launch_cast<0>(vol, f, mode, d_out_rgba, nullptr, nullptr);
+    if ((s = ensure_pool(vol, f.pool_pixels * (mode == VR_MODE_EA ? 4 : 1))) != VR_OK) return s;
+    if ((s = launch_cast<0>(vol, f, mode, vol->d_pool, nullptr, nullptr)) != VR_OK) return s;
+    return launch_composite(vol, f, mode, vol->d_pool, W, H, d_out_rgba, d_out_scalar);
+}
+
+vr_status vr_render_to_host(vr_volume* vol, const vr_camera* cam, int W, int H, float step, int mode, float ert,
+                            float* h_out_rgba) {
+    if (!h_out_rgba) return fail(VR_ERR_INVALID_ARG, "vr_render_to_host: h_out_rgba is NULL");
+    if (!vol) return fail(VR_ERR_INVALID_ARG, "volume is NULL");
+    if (W <= 0 || H <= 0 || W > 32768 || H > 32768) return fail(VR_ERR_INVALID_ARG, "W and H must be in [1,32768]");
+    const size_t floats = (size_t)W * H * 4;
+    if (floats > vol->frame_floats) {
+        if (vol->d_frame) { cudaFree(vol->d_frame); vol->d_frame = nullptr; vol->frame_floats = 0; }
+        VR_CUDA(cudaMalloc(&vol->d_frame, floats * sizeof(float)), "allocate frame");
+        vol->frame_floats = floats;
+    }
+    vr_status s = vr_render(vol, cam, W, H, step, mode, ert, vol->d_frame, nullptr);
+    if (s != VR_OK) return s;
+    VR_CUDA(cudaMemcpyAsync(h_out_rgba, vol->d_frame, floats * sizeof(float), cudaMemcpyDeviceToHost, vol->stream),
+            "copy frame to host");
+    VR_CUDA(cudaStreamSynchronize(vol->stream), "vr_render_to_host");
+    return VR_OK;
+}
+
+vr_status vr_render_bricks(vr_volume* vol, const vr_camera* cam, int W, int H, float step, int mode, float ert,
+                           float* d_brick_images) {
+    vr_status s = check_render_args(vol, cam, W, H, step, mode);
+    if (s != VR_OK) return s;
+    if (!d_brick_images) return fail(VR_ERR_INVALID_ARG, "vr_render_bricks: d_brick_images is NULL");
+    Frame f;
+    build_frame(vol, cam, W, H, step, ert, false, false, f);
+    if ((s = upload_plan(vol, f)) != VR_OK) return s;
+    if (mode == VR_MODE_EA && (s = upload_tf_for_step(vol, (double)step)) != VR_OK) return s;
+    const size_t B = f.recs.size();
+    // full frames: pixels outside a brick's rectangle hold "nothing" (0 / -inf)
+    const size_t n = B * (size_t)W * H * (mode == VR_MODE_EA ? 4 : 1);
+    vr::fill_kernel<<<1184, 256, 0, vol->stream>>>(d_brick_images, n, mode == VR_MODE_EA ? 0.0f : -INFINITY);
+    VR_CUDA(cudaGetLastError(), "fill kernel launch");
+    return launch_cast<0>(vol, f, mode, d_brick_images, nullptr, nullptr);
+}
+
+vr_status vr_composite(vr_volume* vol, const vr_camera* cam, int W, int H, int mode, const float* d_brick_images,
+                       float* d_out_rgba, float* d_out_scalar) {
+    vr_status s = check_render_args(vol, cam, W, H, 1.0f, mode);
+    if (s != VR_OK) return s;
+    if (!d_brick_images || !d_out_rgba) return fail(VR_ERR_INVALID_ARG, "vr_composite: NULL image pointer");
+    Frame f;
+    build_frame(vol, cam, W, H, 1.0f, 0.0f, false, false, f);
+    // a stack of full frames may hold anything anywhere: composite every brick at every pixel
+    for (auto& r : f.recs) { r.rx0 = 0; r.ry0 = 0; r.rw = W; r.rh = H; }
+    if ((s = upload_plan(vol, f)) != VR_OK) return s;
+    return launch_composite(vol, f, mode, d_brick_images, W, H, d_out_rgba, d_out_scalar);
+}
+
+vr_status vr_plan_bricks(const int dims[3], const int bricks[3], const vr_camera* cam, int W, int H,
+                         int out_rect[][4], int out_order[]) {
+    if (!dims || !bricks || !cam || !out_rect || !out_order) return fail(VR_ERR_INVALID_ARG, "vr_plan_bricks: NULL argument");
+    if (W <= 0 || H <= 0) return fail(VR_ERR_INVALID_ARG, "vr_plan_bricks: W and H must be positive");
+    for (int a = 0; a < 3; ++a)
+        if (dims[a] <= 0 || bricks[a] < 1 || bricks[a] > dims[a])
+            return fail(VR_ERR_INVALID_ARG, "vr_plan_bricks: need dims > 0 and 1 <= b_a <= n_a");
+    if ((long long)bricks[0] * bricks[1] * bricks[2] > VR_MAX_BRICKS)
+        return fail(VR_ERR_INVALID_ARG, "vr_plan_bricks: more than VR_MAX_BRICKS bricks");
+    if (const char* why = vr::check_camera(*cam)) return fail(VR_ERR_INVALID_ARG, why);
+    std::vector<vr::BrickPlan> plan;
+    std::vector<int> order;
+    vr::plan_bricks(dims, bricks, *cam, W, H, plan, order);
+    for (size_t b = 0; b < plan.size(); ++b) {
+        out_rect[b][0] = plan[b].rx0; out_rect[b][1] = plan[b].ry0;
+        out_rect[b][2] = plan[b].rw; out_rect[b][3] = plan[b].rh;
+        out_order[b] = order[b];
+    }
+    return VR_OK;
+}
+
+vr_status vr_measure(vr_volume* vol, const vr_camera* cam, int W, int H, float step, int mode, float ert,
+                     long long* h_samples, long long* h_sectors) {
+    vr_status s = check_render_args(vol, cam, W, H, step, mode);
+    if (s != VR_OK) return s;
+    Frame f;
+    build_frame(vol, cam, W, H, step, ert, true, false, f);
+    if ((s = upload_plan(vol, f)) != VR_OK) return s;
+    if (mode == VR_MODE_EA && (s = upload_tf_for_step(vol, (double)step)) != VR_OK) return s;
+    if ((s = ensure_pool(vol, f.pool_pixels * (mode == VR_MODE_EA ? 4 : 1))) != VR_OK) return s;
+    const size_t n_words = (vol->tiled_elems / 8 + 31) / 32;
+    unsigned* d_bitmap = nullptr;
+    unsigned long long* d_cnt = nullptr;
+    VR_CUDA(cudaMalloc(&d_bitmap, n_words * sizeof(unsigned)), "allocate sector bitmap");
+    cudaError_t e = cudaMalloc(&d_cnt, 2 * sizeof(unsigned long long));
+    if (e != cudaSuccess) { cudaFree(d_bitmap); return cuda_fail(e, "allocate counters"); }
+    cudaMemsetAsync(d_bitmap, 0, n_words * sizeof(unsigned), vol->stream);
+    cudaMemsetAsync(d_cnt, 0, 2 * sizeof(unsigned long long), vol->stream);
+    s = launch_cast<1>(vol, f, mode, vol->d_pool, d_cnt, d_bitmap);
+    unsigned long long h[2] = {0, 0};
+    if (s == VR_OK) {
+        vr::popcount_kernel<<<1184, 256, 0, vol->stream>>>(d_bitmap, n_words, d_cnt + 1);
+        e = cudaMemcpyAsync(h, d_cnt, sizeof(h), cudaMemcpyDeviceToHost, vol->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(vol->stream);
+        if (e != cudaSuccess) s = cuda_fail(e, "vr_measure");
+    }
+    cudaFree(d_bitmap);
+    cudaFree(d_cnt);
+    if (s != VR_OK) return s;
+    if (h_samples) *h_samples = (long long)h[0];
+    if (h_sectors) *h_sectors = (long long)h[1];
+    return VR_OK;
+}
+
+vr_status vr_volume_info(const vr_volume* vol, float* h_relayout_ms, long long* h_tiled_bytes) {
+    if (!vol) return fail(VR_ERR_INVALID_ARG, "vr_volume_info: volume is NULL");
+    if (h_relayout_ms) *h_relayout_ms = vol->relayout_ms;
+    if (h_tiled_bytes) *h_tiled_bytes = (long long)(vol->tiled_elems * sizeof(float));
+    return VR_OK;
+}
+
+vr_status vr_export_linear(vr_volume* vol, float* d_linear) {
+    if (!vol || !d_linear) return fail(VR_ERR_INVALID_ARG, "vr_export_linear: NULL argument");
+    vr::export_linear_kernel<<<1184, 256, 0, vol->stream>>>(vol->d_tiled, d_linear, vol->dims[0], vol->dims[1],
+                                                             vol->dims[2], (unsigned)vol->TX * vr::TILE_ELEMS,
+                                                             (unsigned)vol->TX * (unsigned)vol->TY * vr::TILE_ELEMS);
+    VR_CUDA(cudaGetLastError(), "export kernel launch");
+    return VR_OK;
+}
+
+}  // extern "C"

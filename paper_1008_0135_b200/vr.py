@@ -1,0 +1,209 @@
+"""Thin ctypes binding of include/vr.h (libvr_b200.so).  Argument marshalling only.
+
+Same names as the C ABI.  Device buffers are torch CUDA tensors (torch supplies memory and the
+stream; nothing is computed in torch).  Loading fails loudly when the library is missing: there is
+no CPU fallback and nothing here imports oracle/.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libvr_b200.so")
+
+VR_OK, VR_ERR_INVALID_ARG, VR_ERR_STATE, VR_ERR_OOM, VR_ERR_CUDA = 0, 1, 2, 3, 4
+VR_MODE_EA, VR_MODE_MIP = 0, 1
+VR_PROJ_ORTHO, VR_PROJ_PERSP = 0, 1
+VR_MAX_BRICKS = 512
+
+SYMBOLS = ["vr_create_volume", "vr_destroy_volume", "vr_set_stream", "vr_set_transfer_function",
+           "vr_set_bricks", "vr_render", "vr_render_to_host", "vr_render_bricks", "vr_composite",
+           "vr_plan_bricks", "vr_measure", "vr_volume_info", "vr_export_linear", "vr_last_error"]
+
+
+class vr_camera(C.Structure):
+    _fields_ = [("view", C.c_float * 16), ("projection", C.c_int), ("fovy_deg", C.c_float),
+                ("ortho_half_h", C.c_float)]
+
+
+class VrError(RuntimeError):
+    def __init__(self, status, message):
+        super().__init__(f"vr status {status}: {message}")
+        self.status = status
+
+
+_lib = None
+
+
+def lib():
+    """Load libvr_b200.so (built by paper_1008_0135_b200/build.py); raises if it is not there."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_1008_0135_b200.build` "
+                              "(or __graft_entry__.build()); there is no CPU fallback")
+        L = C.CDLL(LIB_PATH)
+        vp, ip, fp = C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_float)
+        cam = C.POINTER(vr_camera)
+        L.vr_create_volume.argtypes = [ip, vp, C.POINTER(vp)]
+        L.vr_destroy_volume.argtypes = [vp]
+        L.vr_destroy_volume.restype = None
+        L.vr_set_stream.argtypes = [vp, vp]
+        L.vr_set_transfer_function.argtypes = [vp, fp, C.c_float, C.c_float]
+        L.vr_set_bricks.argtypes = [vp, C.c_int, C.c_int, C.c_int]
+        L.vr_render.argtypes = [vp, cam, C.c_int, C.c_int, C.c_float, C.c_int, C.c_float, vp, vp]
+        L.vr_render_to_host.argtypes = [vp, cam, C.c_int, C.c_int, C.c_float, C.c_int, C.c_float, vp]
+        L.vr_render_bricks.argtypes = [vp, cam, C.c_int, C.c_int, C.c_float, C.c_int, C.c_float, vp]
+        L.vr_composite.argtypes = [vp, cam, C.c_int, C.c_int, C.c_int, vp, vp, vp]
+        L.vr_plan_bricks.argtypes = [ip, ip, cam, C.c_int, C.c_int, vp, ip]
+        L.vr_measure.argtypes = [vp, cam, C.c_int, C.c_int, C.c_float, C.c_int, C.c_float,
+                                 C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
+        L.vr_volume_info.argtypes = [vp, fp, C.POINTER(C.c_longlong)]
+        L.vr_export_linear.argtypes = [vp, vp]
+        L.vr_last_error.argtypes = []
+        L.vr_last_error.restype = C.c_char_p
+        for name in SYMBOLS:
+            if name not in ("vr_destroy_volume", "vr_last_error"):
+                getattr(L, name).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def vr_last_error():
+    return lib().vr_last_error().decode()
+
+
+def _check(status):
+    if status != VR_OK:
+        raise VrError(status, vr_last_error())
+
+
+def make_camera(view, projection, fovy_deg=45.0, ortho_half_h=1.0):
+    cam = vr_camera()
+    v = np.asarray(view, dtype=np.float32).reshape(16)
+    for i in range(16):
+        cam.view[i] = float(v[i])
+    cam.projection = int(projection)
+    cam.fovy_deg = float(fovy_deg)
+    cam.ortho_half_h = float(ortho_half_h)
+    return cam
+
+
+def camera_from_spec(cs):
+    """cs: workloads.CameraSpec (or anything with view/projection/fovy_deg/ortho_half_h)."""
+    return make_camera(cs.view, cs.projection, cs.fovy_deg, cs.ortho_half_h)
+
+
+def _i3(a):
+    return (C.c_int * 3)(*[int(x) for x in a])
+
+
+def _dptr(t, dtype_name="float32"):
+    """Device pointer of a contiguous torch CUDA tensor (None -> NULL)."""
+    if t is None:
+        return None
+    import torch
+    assert isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous(), "need a contiguous CUDA tensor"
+    assert str(t.dtype) == "torch." + dtype_name, f"need {dtype_name}"
+    return C.c_void_p(t.data_ptr())
+
+
+def vr_plan_bricks(dims, bricks, cam, W, H):
+    """Host-only: (rects [B,4] = x0,y0,w,h ; order [B] front to back)."""
+    B = int(bricks[0]) * int(bricks[1]) * int(bricks[2])
+    rect = np.zeros((max(B, 1), 4), dtype=np.int32)
+    order = np.zeros(max(B, 1), dtype=np.int32)
+    _check(lib().vr_plan_bricks(_i3(dims), _i3(bricks), C.byref(cam), int(W), int(H),
+                                rect.ctypes.data_as(C.c_void_p), order.ctypes.data_as(C.POINTER(C.c_int))))
+    return rect[:B], order[:B]
+
+
+class Volume:
+    """Owner of one vr_volume handle.  `cube` is a torch float32 CUDA tensor of shape (nz,ny,nx)."""
+
+    def __init__(self, cube, stream=None):
+        import torch
+        assert cube.dim() == 3
+        self.dims = (int(cube.shape[2]), int(cube.shape[1]), int(cube.shape[0]))
+        self.device = cube.device
+        self.bricks = (1, 1, 1)
+        self._h = C.c_void_p()
+        with torch.cuda.device(self.device):
+            torch.cuda.current_stream().synchronize()      # the cube must be complete: a0 runs on stream 0
+            _check(lib().vr_create_volume(_i3(self.dims), _dptr(cube), C.byref(self._h)))
+            self.vr_set_stream(torch.cuda.current_stream() if stream is None else stream)
+
+    def close(self):
+        if self._h:
+            lib().vr_destroy_volume(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- same names as the C ABI ------------------------------------------------------------------
+    def vr_set_stream(self, stream):
+        _check(lib().vr_set_stream(self._h, C.c_void_p(stream.cuda_stream)))
+
+    def vr_set_transfer_function(self, rgba, vmin, vmax):
+        t = np.ascontiguousarray(rgba, dtype=np.float32).reshape(1024)
+        _check(lib().vr_set_transfer_function(self._h, t.ctypes.data_as(C.POINTER(C.c_float)),
+                                              float(vmin), float(vmax)))
+
+    def vr_set_bricks(self, bx, by, bz):
+        _check(lib().vr_set_bricks(self._h, int(bx), int(by), int(bz)))
+        self.bricks = (int(bx), int(by), int(bz))
+
+    def vr_render(self, cam, W, H, step, mode, ert_alpha=0.0, out=None, out_scalar=None):
+        import torch
+        if out is None:
+            out = torch.empty((H, W, 4), dtype=torch.float32, device=self.device)
+        _check(lib().vr_render(self._h, C.byref(cam), int(W), int(H), float(step), int(mode),
+                               float(ert_alpha), _dptr(out), _dptr(out_scalar)))
+        return out
+
+    def vr_render_to_host(self, cam, W, H, step, mode, ert_alpha, host_out):
+        """host_out: torch CPU float32 tensor [H,W,4] (pinned for an asynchronous copy)."""
+        assert not host_out.is_cuda and host_out.is_contiguous() and host_out.numel() == H * W * 4
+        _check(lib().vr_render_to_host(self._h, C.byref(cam), int(W), int(H), float(step), int(mode),
+                                       float(ert_alpha), C.c_void_p(host_out.data_ptr())))
+        return host_out
+
+    def vr_render_bricks(self, cam, W, H, step, mode, ert_alpha=0.0):
+        import torch
+        B = self.bricks[0] * self.bricks[1] * self.bricks[2]
+        shape = (B, H, W, 4) if mode == VR_MODE_EA else (B, H, W)
+        imgs = torch.empty(shape, dtype=torch.float32, device=self.device)
+        _check(lib().vr_render_bricks(self._h, C.byref(cam), int(W), int(H), float(step), int(mode),
+                                      float(ert_alpha), _dptr(imgs)))
+        return imgs
+
+    def vr_composite(self, cam, W, H, mode, brick_images, out=None, out_scalar=None):
+        import torch
+        if out is None:
+            out = torch.empty((H, W, 4), dtype=torch.float32, device=self.device)
+        _check(lib().vr_composite(self._h, C.byref(cam), int(W), int(H), int(mode), _dptr(brick_images),
+                                  _dptr(out), _dptr(out_scalar)))
+        return out
+
+    def vr_measure(self, cam, W, H, step, mode, ert_alpha=0.0):
+        """(samples evaluated, distinct 32-byte sectors touched) from the instrumented caster."""
+        s, k = C.c_longlong(0), C.c_longlong(0)
+        _check(lib().vr_measure(self._h, C.byref(cam), int(W), int(H), float(step), int(mode),
+                                float(ert_alpha), C.byref(s), C.byref(k)))
+        return s.value, k.value
+
+    def vr_volume_info(self):
+        ms, nb = C.c_float(0), C.c_longlong(0)
+        _check(lib().vr_volume_info(self._h, C.byref(ms), C.byref(nb)))
+        return ms.value, nb.value
+
+    def vr_export_linear(self):
+        import torch
+        out = torch.empty((self.dims[2], self.dims[1], self.dims[0]), dtype=torch.float32, device=self.device)
+        _check(lib().vr_export_linear(self._h, _dptr(out)))
+        return out
