@@ -1,0 +1,370 @@
+#!/usr/bin/env python
+"""bench.py — ms/frame of the whole hot path (per-brick ray casting + sort-last composite) at 1024^2
+on the GASS-sized 2048x2048x1600 float32 cube (26.8 GB), BASELINE.json configs[3]: 2x2x2 bricks,
+perspective 45 deg, step 1 voxel, early termination at alpha 0.995, 36-view orbit about the y axis.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 0..3]
+
+A step is one frame (one view of the orbit; view k uses azimuth 10*(k mod 36) degrees).  The cube is
+synthetic (workloads.cube_gass_like, seed 3), generated on the device, re-laid once by
+vr_create_volume (reported separately as `relayout`, a load-time cost like the paper's file load,
+PAPER.md:136) and then resident in HBM.  The cube is 26.8 GB >> the 126 MB L2, so nothing survives
+between frames and no L2 flush is needed.  N > 1: replicas only — every
+rank holds the whole cube and renders its own K frames of the orbit; no data-path collective.
+
+--impl reference times the CPU oracle (oracle/, double precision, OpenMP) on the host cores on the
+same workload; each step renders every 4th pixel in x and y of the frame and scales the time by 16.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+import torch
+
+from paper_1008_0135_b200 import workloads as wl
+
+METRIC = "ms_per_frame_1024x1024"
+UNIT = "ms/frame"
+# Per-launch DRAM traffic of cast_kernel<EA> from the committed `ncu --set full` capture
+# (dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01_cast_full.md); None until captured.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+
+
+def env_int(name, default):
+    try:
+        return int(os.environ.get(name, default))
+    except ValueError:
+        return default
+
+
+def measured_peak_gbs():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons of one GPU, sampled every 200 ms while running."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [l for (t, l) in self.lines if t0 - 0.1 <= t <= t1 + 0.3] or [l for (_, l) in self.lines]
+        for l in rows:
+            f = [x.strip() for x in l.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def workload_for(args):
+    w = wl.config(args.config)
+    views = wl.orbit_azimuths() if args.config == 3 else [w.az_deg]
+    return w, views
+
+
+def describe(w, views):
+    B = w.bricks[0] * w.bricks[1] * w.bricks[2]
+    return {"workload": w.name, "cube": "x".join(str(d) for d in w.dims) + " f32", "seed": w.seed,
+            "cube_GB": round(4e-9 * w.dims[0] * w.dims[1] * w.dims[2], 2), "bricks": "x".join(map(str, w.bricks)),
+            "n_bricks": B, "image": f"{w.W}x{w.H}", "projection": "perspective45" if w.projection else "orthographic",
+            "step_voxels": w.step, "mode": "EA" if w.mode == 0 else "MIP", "ert_alpha": w.ert_alpha,
+            "views": f"{len(views)}-view orbit about y, el {w.el_deg} deg" if len(views) > 1 else f"az {w.az_deg} el {w.el_deg}",
+            "l2": "cube >> 126 MB L2: inputs larger than L2, no flush" if w.dims[0] * w.dims[1] * w.dims[2] * 4 > 4e8
+                  else "cube fits L2; 512 MB scratch written between frames to flush it"}
+
+
+# ------------------------------------------------------------------------------------------------
+def run_ours(args):
+    from paper_1008_0135_b200 import vr                      # fails loudly without the CUDA library
+    vr.lib()
+    rank, world = env_int("RANK", 0), env_int("WORLD_SIZE", 1)
+    local = env_int("LOCAL_RANK", 0)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w, views = workload_for(args)
+    K, Wm = args.steps, args.warmup
+    cube = w.cube("cuda")
+    torch.cuda.synchronize()
+    vol = vr.Volume(cube)
+    relayout_ms, tiled_bytes = vol.vr_volume_info()
+    vol.vr_set_transfer_function(w.table, w.vmin, w.vmax)
+    vol.vr_set_bricks(*w.bricks)
+    B = w.bricks[0] * w.bricks[1] * w.bricks[2]
+    cams = [vr.camera_from_spec(w.camera(az_deg=a)) for a in views]
+    out = torch.empty((w.H, w.W, 4), dtype=torch.float32, device="cuda")
+    small = w.dims[0] * w.dims[1] * w.dims[2] * 4 <= 4e8
+    scratch = torch.empty(128 << 20, dtype=torch.float32, device="cuda") if small else None
+
+    def view_of(step_idx):
+        # ranks start at different points of the orbit (replicas render different views)
+        return (step_idx + rank * max(1, len(views) // world)) % len(views)
+
+    def frame(k):
+        if scratch is not None:
+            scratch.fill_(float(k))                              # L2 flush (outside the per-frame events)
+        vol.vr_render(cams[view_of(k)], w.W, w.H, w.step, w.mode, w.ert_alpha, out=out)
+
+    for k in range(Wm):
+        frame(k)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    time.sleep(0.3)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * K)]
+    cast_ms, comp_ms = [], []
+    barrier()
+    t_wall0 = time.time()
+    for k in range(K):
+        if scratch is not None:
+            scratch.fill_(float(k))
+        ev[2 * k].record()
+        vol.vr_render(cams[view_of(k)], w.W, w.H, w.step, w.mode, w.ert_alpha, out=out)
+        ev[2 * k + 1].record()
+        if args.stage_times:                                      # waits for the frame: off by default
+            c, m = vol.vr_get_stage_ms()
+            cast_ms.append(c); comp_ms.append(m)
+    barrier()
+    t_wall1 = time.time()
+    clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
+    per_frame = [ev[2 * k].elapsed_time(ev[2 * k + 1]) for k in range(K)]
+    total_ms = ev[0].elapsed_time(ev[2 * K - 1]) if scratch is None else float(sum(per_frame))
+    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+
+    # ---- stage split: second, untimed-for-the-headline pass with the library's own events ----
+    for k in range(K):
+        if scratch is not None:
+            scratch.fill_(float(k))
+        vol.vr_render(cams[view_of(k)], w.W, w.H, w.step, w.mode, w.ert_alpha, out=out)
+        c, m = vol.vr_get_stage_ms()
+        cast_ms.append(c); comp_ms.append(m)
+
+    # ---- end to end through the public call with a HOST frame buffer (pinned), D2H inside ----
+    host_out = torch.empty((w.H, w.W, 4), dtype=torch.float32).pin_memory()
+    for k in range(min(Wm, 3)):
+        vol.vr_render_to_host(cams[view_of(k)], w.W, w.H, w.step, w.mode, w.ert_alpha, host_out)
+    barrier()
+    t0 = time.perf_counter()
+    for k in range(K):
+        if scratch is not None:
+            scratch.fill_(float(k))
+        vol.vr_render_to_host(cams[view_of(k)], w.W, w.H, w.step, w.mode, w.ert_alpha, host_out)
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3
+    t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_ms = float(t.item())
+
+    if rank != 0:
+        if dist is not None:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
+
+    # ---- untimed instrumented pass: samples evaluated and distinct 32-byte sectors per view ----
+    used_views = sorted(set(view_of(k) for k in range(K)))
+    meas = {}
+    for v in used_views:
+        meas[v] = vol.vr_measure(cams[v], w.W, w.H, w.step, w.mode, w.ert_alpha)
+    samples = sum(meas[view_of(k)][0] for k in range(K))
+    alg_bytes = 32.0 * sum(meas[view_of(k)][1] for k in range(K))
+    cast_total_ms = float(sum(cast_ms))
+    peak, peak_src = measured_peak_gbs()
+    achieved = alg_bytes / (cast_total_ms * 1e-3) / 1e9
+    ms_per_frame = total_ms / K
+
+    # ---- the oracle beside it: one full frame (view az 30 deg) on the host cores ----
+    cpu = None
+    parity = None
+    if not args.no_cpu_baseline:
+        from oracle import vro                                    # cpu_baseline leg only
+        host_cube = cube.cpu().numpy()
+        az = 30.0
+        cs = w.camera(az_deg=az)
+        ocam = vro.make_camera(cs.view, cs.projection, cs.fovy_deg, cs.ortho_half_h)
+        stride = args.cpu_stride
+        xs = np.arange(0, w.W, stride, dtype=np.int32)
+        ys = np.arange(0, w.H, stride, dtype=np.int32)
+        yy, xx = np.meshgrid(ys, xs, indexing="ij")
+        t0 = time.perf_counter()
+        ref = vro.render_pixels(host_cube, w.table, w.vmin, w.vmax, w.bricks, ocam, w.W, w.H, w.step, w.mode,
+                                w.ert_alpha, 1, xx.reshape(-1), yy.reshape(-1))
+        cpu_s = time.perf_counter() - t0
+        frac = xx.size / float(w.W * w.H)
+        cpu = {"value": cpu_s * 1e3 / frac, "unit": UNIT, "cores": vro.max_threads(), "kind": "oracle",
+               "sample": f"view az {az:g} deg, every {stride}th pixel in x and y ({xx.size} rays, "
+                         f"{ref['samples']} samples, {cpu_s:.1f} s of wall time), scaled by {1 / frac:g}",
+               "msamples_per_s": ref["samples"] / cpu_s / 1e6}
+        got = vol.vr_render(vr.camera_from_spec(cs), w.W, w.H, w.step, w.mode, w.ert_alpha)
+        torch.cuda.synchronize()
+        g = got.cpu().numpy()[::stride, ::stride].reshape(-1, 4)
+        parity = {"max_abs_err_vs_oracle": float(np.abs(g - ref["rgba"]).max()), "pixels": int(xx.size),
+                  "gate": 5e-3 if w.ert_alpha > 0 else 1e-4}
+        del host_cube
+
+    line = {
+        "metric": METRIC, "value": ms_per_frame, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+        "ms_per_step": ms_per_frame, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic", "config": describe(w, views),
+        "frames_per_s_all_gpus": world * K / (total_ms * 1e-3),
+        "ms_per_frame_min": min(per_frame), "ms_per_frame_max": max(per_frame),
+        "ms_per_view": {str(int(views[view_of(k)])): round(per_frame[k], 3) for k in range(K)},
+        "gsamples_per_s": samples / (total_ms * 1e-3) / 1e9 * world,
+        "samples_per_frame": samples / K,
+        "stages_ms": {"cast": cast_total_ms / K, "composite": float(sum(comp_ms)) / K},
+        "relayout": {"ms": relayout_ms, "GBps_read_plus_write": (4.0 * cube.numel() + tiled_bytes) / (relayout_ms * 1e-3) / 1e9
+                     if relayout_ms > 0 else None},
+        "clocks": clocks,
+        "e2e": {"value": e2e_ms / K, "unit": UNIT, "h2d_bytes_per_step": B * (72 + 4) + 256,
+                "d2h_bytes_per_step": w.W * w.H * 16,
+                "note": "vr_render_to_host: per-frame plan upload + kernels + D2H of the RGBA frame into pinned host memory"},
+        "gpu_launches": 2 * K if B > 1 or w.mode == 1 else K,
+        "roofline": {"bound": "hbm", "kernel": "cast_kernel<EA>" if w.mode == 0 else "cast_kernel<MIP>",
+                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH, "peak_source": peak_src,
+                     "algorithmic_bytes_per_launch": alg_bytes / K,
+                     "cube_bytes": 4.0 * cube.numel(), "avg_launch_ms": cast_total_ms / K,
+                     "definition": "32 B x distinct sectors of the tiled cube touched by the frame's samples "
+                                   "(instrumented pass, untimed) / cast kernel time (CUDA events)"},
+        "cpu_baseline": cpu, "parity": parity,
+        "paper_context": "< 0.3 s per 1024^2 frame of the 26 GB GASS cube on 3 workstations / 8 Tesla C1060 "
+                         "(PAPER.md:9,304): another machine and the real cube, context only",
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+# ------------------------------------------------------------------------------------------------
+def run_reference(args):
+    """The oracle as it stands, timed on the host cores (rank 0 only)."""
+    if env_int("RANK", 0) != 0:
+        return
+    from oracle import vro
+    w, views = workload_for(args)
+    K, Wm = args.steps, args.warmup
+    dev = "cuda" if torch.cuda.is_available() else "cpu"         # generation only; not timed
+    host_cube = w.cube(dev).cpu().numpy()
+    stride = args.cpu_stride
+    xs = np.arange(0, w.W, stride, dtype=np.int32)
+    ys = np.arange(0, w.H, stride, dtype=np.int32)
+    yy, xx = np.meshgrid(ys, xs, indexing="ij")
+    px, py = xx.reshape(-1), yy.reshape(-1)
+    frac = px.size / float(w.W * w.H)
+
+    def step(k):
+        cs = w.camera(az_deg=views[k % len(views)])
+        ocam = vro.make_camera(cs.view, cs.projection, cs.fovy_deg, cs.ortho_half_h)
+        return vro.render_pixels(host_cube, w.table, w.vmin, w.vmax, w.bricks, ocam, w.W, w.H, w.step, w.mode,
+                                 w.ert_alpha, 1, px, py)["samples"]
+
+    for k in range(Wm):
+        step(k)
+    t0 = time.perf_counter()
+    samples = 0
+    for k in range(K):
+        samples += step(k)
+    dt = time.perf_counter() - t0
+    ms = dt * 1e3 / K / frac
+    sample = (f"each step: every {stride}th pixel in x and y of one orbit view ({px.size} rays), time scaled by "
+              f"{1 / frac:g} to a full frame")
+    line = {"impl": "reference", "metric": METRIC, "value": ms, "unit": UNIT, "n_gpus": args.gpus, "steps": K,
+            "warmup": Wm, "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": describe(w, views),
+            "cpu_baseline": {"value": ms, "unit": UNIT, "kind": "oracle", "cores": vro.max_threads(), "sample": sample,
+                             "msamples_per_s": samples / dt / 1e6},
+            "e2e": {"value": ms, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=36)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (0..3); 3 is the headline")
+    ap.add_argument("--cpu-stride", type=int, default=None,
+                    help="oracle legs render every n-th pixel in x and y (default 1 = the full frame for cpu_baseline, 4 for --impl reference)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--stage-times", action="store_true", help=argparse.SUPPRESS)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.cpu_stride is None:
+        args.cpu_stride = 4 if args.impl == "reference" else 1
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -124,6 +124,10 @@ vr_status vr_plan_bricks(const int dims[3], const int bricks[3], const vr_camera
  *     Synchronises.  Either output may be NULL.                                                  */
 vr_status vr_measure(vr_volume* vol, const vr_camera* cam, int W, int H, float step_voxels, int mode,
                      float ert_alpha, long long* h_samples, long long* h_sectors);
+/* Device time, in ms, of the cast kernel and of the composite kernel of the most recent vr_render /
+ *     vr_render_to_host on this volume (CUDA events recorded on the volume's stream around each
+ *     launch; composite is 0 when a single brick wrote the frame directly).  Waits for that frame. */
+vr_status vr_get_stage_ms(vr_volume* vol, float* h_cast_ms, float* h_composite_ms);
 /* Device time of the re-layout kernel of vr_create_volume, in ms, and the bytes it allocated.  */
 vr_status vr_volume_info(const vr_volume* vol, float* h_relayout_ms, long long* h_tiled_bytes);
 /* Inverse of the re-layout: gathers the tiled copy back into d_linear[nz][ny][nx] (round-trip test). */

@@ -57,6 +57,9 @@ struct vr_volume {
     size_t pool_floats = 0;
     float* d_frame = nullptr;         // internal frame of vr_render_to_host
     size_t frame_floats = 0;
+
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};   // cast begin/end, composite begin/end
+    bool timed_cast = false, timed_comp = false;
 };
 
 namespace {
@@ -236,6 +239,7 @@ vr_status vr_create_volume(const int dims[3], const float* d_data, vr_volume** o
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (e == cudaSuccess) e = cudaEventCreate(&e0);
     if (e == cudaSuccess) e = cudaEventCreate(&e1);
+    for (int k = 0; k < 4 && e == cudaSuccess; ++k) e = cudaEventCreate(&v->ev[k]);
     if (e == cudaSuccess) {
         dim3 grid((v->TX + 7) / 8, v->TY, v->TZ);
         cudaEventRecord(e0, v->stream);
@@ -265,6 +269,8 @@ void vr_destroy_volume(vr_volume* v) {
     if (v->d_order) cudaFree(v->d_order);
     if (v->d_pool) cudaFree(v->d_pool);
     if (v->d_frame) cudaFree(v->d_frame);
+    for (int k = 0; k < 4; ++k)
+        if (v->ev[k]) cudaEventDestroy(v->ev[k]);
     delete v;
 }
 
@@ -311,10 +317,31 @@ vr_status vr_render(vr_volume* vol, const vr_camera* cam, int W, int H, float st
     build_frame(vol, cam, W, H, step, ert, true, direct, f);
     if ((s = upload_plan(vol, f)) != VR_OK) return s;
     if (mode == VR_MODE_EA && (s = upload_tf_for_step(vol, (double)step)) != VR_OK) return s;
-    if (direct) return launch_cast<0>(vol, f, mode, d_out_rgba, nullptr, nullptr);
-    if ((s = ensure_pool(vol, f.pool_pixels * (mode == VR_MODE_EA ? 4 : 1))) != VR_OK) return s;
-    if ((s = launch_cast<0>(vol, f, mode, vol->d_pool, nullptr, nullptr)) != VR_OK) return s;
-    return launch_composite(vol, f, mode, vol->d_pool, W, H, d_out_rgba, d_out_scalar);
+    vol->timed_cast = vol->timed_comp = false;
+    if (!direct && (s = ensure_pool(vol, f.pool_pixels * (mode == VR_MODE_EA ? 4 : 1))) != VR_OK) return s;
+    cudaEventRecord(vol->ev[0], vol->stream);
+    s = launch_cast<0>(vol, f, mode, direct ? d_out_rgba : vol->d_pool, nullptr, nullptr);
+    cudaEventRecord(vol->ev[1], vol->stream);
+    if (s != VR_OK) return s;
+    vol->timed_cast = true;
+    if (direct) return VR_OK;
+    cudaEventRecord(vol->ev[2], vol->stream);
+    s = launch_composite(vol, f, mode, vol->d_pool, W, H, d_out_rgba, d_out_scalar);
+    cudaEventRecord(vol->ev[3], vol->stream);
+    if (s == VR_OK) vol->timed_comp = true;
+    return s;
+}
+
+vr_status vr_get_stage_ms(vr_volume* vol, float* h_cast_ms, float* h_composite_ms) {
+    if (!vol) return fail(VR_ERR_INVALID_ARG, "vr_get_stage_ms: volume is NULL");
+    if (!vol->timed_cast) return fail(VR_ERR_STATE, "vr_get_stage_ms: no frame rendered yet");
+    float c = 0.f, m = 0.f;
+    VR_CUDA(cudaEventSynchronize(vol->ev[vol->timed_comp ? 3 : 1]), "vr_get_stage_ms");
+    VR_CUDA(cudaEventElapsedTime(&c, vol->ev[0], vol->ev[1]), "vr_get_stage_ms");
+    if (vol->timed_comp) VR_CUDA(cudaEventElapsedTime(&m, vol->ev[2], vol->ev[3]), "vr_get_stage_ms");
+    if (h_cast_ms) *h_cast_ms = c;
+    if (h_composite_ms) *h_composite_ms = m;
+    return VR_OK;
 }
 
 vr_status vr_render_to_host(vr_volume* vol, const vr_camera* cam, int W, int H, float step, int mode, float ert,

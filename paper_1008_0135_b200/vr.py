@@ -19,7 +19,7 @@ VR_MAX_BRICKS = 512
 
 SYMBOLS = ["vr_create_volume", "vr_destroy_volume", "vr_set_stream", "vr_set_transfer_function",
            "vr_set_bricks", "vr_render", "vr_render_to_host", "vr_render_bricks", "vr_composite",
-           "vr_plan_bricks", "vr_measure", "vr_volume_info", "vr_export_linear", "vr_last_error"]
+           "vr_plan_bricks", "vr_measure", "vr_get_stage_ms", "vr_volume_info", "vr_export_linear", "vr_last_error"]
 
 
 class vr_camera(C.Structure):
@@ -59,6 +59,7 @@ def lib():
         L.vr_plan_bricks.argtypes = [ip, ip, cam, C.c_int, C.c_int, vp, ip]
         L.vr_measure.argtypes = [vp, cam, C.c_int, C.c_int, C.c_float, C.c_int, C.c_float,
                                  C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
+        L.vr_get_stage_ms.argtypes = [vp, fp, fp]
         L.vr_volume_info.argtypes = [vp, fp, C.POINTER(C.c_longlong)]
         L.vr_export_linear.argtypes = [vp, vp]
         L.vr_last_error.argtypes = []
@@ -196,6 +197,12 @@ class Volume:
         _check(lib().vr_measure(self._h, C.byref(cam), int(W), int(H), float(step), int(mode),
                                 float(ert_alpha), C.byref(s), C.byref(k)))
         return s.value, k.value
+
+    def vr_get_stage_ms(self):
+        """(cast ms, composite ms) of the most recent vr_render; waits for it."""
+        a, b = C.c_float(0), C.c_float(0)
+        _check(lib().vr_get_stage_ms(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
 
     def vr_volume_info(self):
         ms, nb = C.c_float(0), C.c_longlong(0)
