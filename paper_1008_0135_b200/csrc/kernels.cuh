@@ -208,6 +208,10 @@ __device__ __forceinline__ float trilerp(const Footprint& F) {
     return fmaf(F.fz, c1 - c0, c0);
 }
 
+}  // namespace vr
+#include "sampler.cuh"
+namespace vr {
+
 // O6 + O7: classify through the shared-memory table (entry m: T[m], then T[m+1]-T[m]) and blend.
 __device__ __forceinline__ void classify_blend(const float4* __restrict__ tf, const FrameParams& P, float value,
                                                float& Cr, float& Cg, float& Cb, float& A) {
@@ -322,26 +326,31 @@ cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ 
         }
         if (counters) atomicAdd(counters, count);
     } else {
-        // two samples in flight per iteration: 16 independent loads before the first blend
-        for (int j = 0; j < n; j += 2) {
-            const float j0 = (float)j, j1 = (float)(j + 1);
-            Footprint F0, F1;
-            fetch<0>(vol, P, nxm1, nym1, nzm1, fmaf(j0, hx, fmaf(j0, ex, q0x)), fmaf(j0, hy, fmaf(j0, ey, q0y)),
-                     fmaf(j0, hz, fmaf(j0, ez, q0z)), F0, nullptr);
-            fetch<0>(vol, P, nxm1, nym1, nzm1, fmaf(j1, hx, fmaf(j1, ex, q0x)), fmaf(j1, hy, fmaf(j1, ey, q0y)),
-                     fmaf(j1, hz, fmaf(j1, ez, q0z)), F1, nullptr);
-            const float v0 = trilerp(F0), v1 = trilerp(F1);
+        // Row-cached sampler (sampler.cuh); the blend of sample j-1 is issued after the loads of sample j
+        // so that classification and blending overlap the load latency.
+        RowCache K;
+        K.have = false; K.prev_straddle = false; K.cx = 0; K.iy = 0; K.iz = 0;
+        K.e[0][0] = K.e[0][1] = K.e[1][0] = K.e[1][1] = 0.0f;
+        K.r[0][0] = K.r[0][1] = K.r[1][0] = K.r[1][1] = make_float4(0.f, 0.f, 0.f, 0.f);
+        const bool ypos = dsy >= 0.0, zpos = dsz >= 0.0;
+        float vprev = sample_cached(vol, P.ty_stride, P.slab_stride, nxm1, nym1, nzm1, q0x, q0y, q0z, ypos, zpos, K);
+        bool done = false;
+        for (int j = 1; j < n; ++j) {
+            const float jf = (float)j;
+            const float v = sample_cached(vol, P.ty_stride, P.slab_stride, nxm1, nym1, nzm1,
+                                          fmaf(jf, hx, fmaf(jf, ex, q0x)), fmaf(jf, hy, fmaf(jf, ey, q0y)),
+                                          fmaf(jf, hz, fmaf(jf, ez, q0z)), ypos, zpos, K);
             if (MODE == MODE_EA) {
-                classify_blend(tf, P, v0, Cr, Cg, Cb, A);
-                if (P.ert_on && A >= P.ert) break;
-                if (j + 1 < n) {
-                    classify_blend(tf, P, v1, Cr, Cg, Cb, A);
-                    if (P.ert_on && A >= P.ert) break;
-                }
+                classify_blend(tf, P, vprev, Cr, Cg, Cb, A);
+                if (P.ert_on && A >= P.ert) { done = true; break; }
             } else {
-                M = fmaxf(M, v0);
-                if (j + 1 < n) M = fmaxf(M, v1);
+                M = fmaxf(M, vprev);
             }
+            vprev = v;
+        }
+        if (!done) {
+            if (MODE == MODE_EA) classify_blend(tf, P, vprev, Cr, Cg, Cb, A);
+            else M = fmaxf(M, vprev);
         }
     }
     if (MODE == MODE_EA) reinterpret_cast<float4*>(img)[pix] = make_float4(Cr, Cg, Cb, A);
