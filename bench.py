@@ -30,6 +30,7 @@ if ROOT not in sys.path:
 import numpy as np
 import torch
 
+from paper_1008_0135_b200 import replicas
 from paper_1008_0135_b200 import workloads as wl
 
 METRIC = "ms_per_frame_1024x1024"
@@ -159,7 +160,7 @@ def run_ours(args):
 
     def view_of(step_idx):
         # ranks start at different points of the orbit (replicas render different views)
-        return (step_idx + rank * max(1, len(views) // world)) % len(views)
+        return replicas.view_of(step_idx, rank, world, len(views))
 
     def frame(k):
         if scratch is not None:
@@ -191,10 +192,7 @@ def run_ours(args):
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
     per_frame = [ev[2 * k].elapsed_time(ev[2 * k + 1]) for k in range(K)]
     total_ms = ev[0].elapsed_time(ev[2 * K - 1]) if scratch is None else float(sum(per_frame))
-    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
+    total_ms = replicas.max_over_ranks(total_ms, dist, "cuda")
 
     # ---- stage split: second, untimed-for-the-headline pass with the library's own events ----
     for k in range(K):
@@ -216,10 +214,7 @@ def run_ours(args):
         vol.vr_render_to_host(cams[view_of(k)], w.W, w.H, w.step, w.mode, w.ert_alpha, host_out)
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - t0) * 1e3
-    t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_ms = float(t.item())
+    e2e_ms = replicas.max_over_ranks(e2e_ms, dist, "cuda")
 
     if rank != 0:
         if dist is not None:
@@ -237,7 +232,7 @@ def run_ours(args):
     cast_total_ms = float(sum(cast_ms))
     peak, peak_src = measured_peak_gbs()
     achieved = alg_bytes / (cast_total_ms * 1e-3) / 1e9
-    ms_per_frame = total_ms / K
+    ms_per_frame = replicas.aggregate_ms_per_frame(total_ms, K, world)   # whole job: all ranks' frames
 
     # ---- the oracle beside it: one full frame (view az 30 deg) on the host cores ----
     cpu = None
@@ -270,7 +265,7 @@ def run_ours(args):
 
     line = {
         "metric": METRIC, "value": ms_per_frame, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
-        "ms_per_step": ms_per_frame, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": total_ms / K, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic", "config": describe(w, views),
         "frames_per_s_all_gpus": world * K / (total_ms * 1e-3),
         "ms_per_frame_min": min(per_frame), "ms_per_frame_max": max(per_frame),
@@ -281,7 +276,7 @@ def run_ours(args):
         "relayout": {"ms": relayout_ms, "GBps_read_plus_write": (4.0 * cube.numel() + tiled_bytes) / (relayout_ms * 1e-3) / 1e9
                      if relayout_ms > 0 else None},
         "clocks": clocks,
-        "e2e": {"value": e2e_ms / K, "unit": UNIT, "h2d_bytes_per_step": B * (72 + 4) + 256,
+        "e2e": {"value": replicas.aggregate_ms_per_frame(e2e_ms, K, world), "unit": UNIT, "h2d_bytes_per_step": B * (72 + 4) + 256,
                 "d2h_bytes_per_step": w.W * w.H * 16,
                 "note": "vr_render_to_host: per-frame plan upload + kernels + D2H of the RGBA frame into pinned host memory"},
         "gpu_launches": 2 * K if B > 1 or w.mode == 1 else K,
