@@ -130,6 +130,11 @@ vr_status vr_measure(vr_volume* vol, const vr_camera* cam, int W, int H, float s
 vr_status vr_get_stage_ms(vr_volume* vol, float* h_cast_ms, float* h_composite_ms);
 /* Device time of the re-layout kernel of vr_create_volume, in ms, and the bytes it allocated.  */
 vr_status vr_volume_info(const vr_volume* vol, float* h_relayout_ms, long long* h_tiled_bytes);
+/* Minimum and maximum of the cube (NaN voxels ignored), computed by the re-layout pass of vr_create_volume at
+ *     no extra memory traffic: the data range a transfer function is set over when the file metadata does not
+ *     give one ("each GPU computes the minimum and maximum of its portion").
+ *     STATE if every voxel is NaN.                                                               */
+vr_status vr_volume_range(const vr_volume* vol, float* h_min, float* h_max);
 /* Inverse of the re-layout: gathers the tiled copy back into d_linear[nz][ny][nx] (round-trip test). */
 vr_status vr_export_linear(vr_volume* vol, float* d_linear);
 

@@ -10,13 +10,24 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <string.h>
 
 namespace vr {
 
 constexpr int TILE = 8;                 // voxels per tile edge
 constexpr int TILE_ELEMS = 512;         // 8^3 floats = 2 KB, x-rows of 32 B = one DRAM sector
-constexpr int CTA_PX = 16;              // a CTA renders a 16x16-pixel tile: 8 warps of 8x4 pixels
-constexpr int CTA_THREADS = 256;
+// CTA shape of the caster, chosen by measurement on the config-3 orbit (B200): 16x8 pixels (4 warps) with 7
+// CTAs per SM (72 registers) gave 5.88 ms mean cast time; 16x16 with 3 CTAs 6.08 ms; forcing 64 registers for
+// 8 CTAs (32 warps) 7.6 ms - more resident rays thrash the L1 that carries the sector re-use between rays.
+#ifndef VR_CTA_H
+#define VR_CTA_H 8
+#endif
+#ifndef VR_CAST_MINBLOCKS
+#define VR_CAST_MINBLOCKS 7
+#endif
+constexpr int CTA_W = 16;               // a CTA renders a CTA_W x CTA_H pixel tile: warps of 8x4 pixels, 2 across
+constexpr int CTA_H = VR_CTA_H;
+constexpr int CTA_THREADS = CTA_W * CTA_H;
 constexpr int MODE_EA = 0, MODE_MIP = 1;
 
 struct FrameParams {
@@ -48,22 +59,65 @@ struct BrickRec {
 // x+1 / y+1 / z+1 of any in-range voxel addressable without a bounds test, with the same result as
 // the clamp of O5 because the weight of the replicated voxel is then exactly zero).
 // ------------------------------------------------------------------------------------------------
+constexpr int RANGE_SLOTS = 256;
+// order-preserving map float -> unsigned (so atomicMin/atomicMax on the key order the floats)
+__host__ __device__ __forceinline__ unsigned float_key(float f) {
+#ifdef __CUDA_ARCH__
+    const unsigned u = __float_as_uint(f);
+#else
+    unsigned u; memcpy(&u, &f, 4);
+#endif
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__host__ __device__ __forceinline__ float key_float(unsigned k) {
+    const unsigned u = (k & 0x80000000u) ? (k & 0x7fffffffu) : ~k;
+#ifdef __CUDA_ARCH__
+    return __uint_as_float(u);
+#else
+    float f; memcpy(&f, &u, 4); return f;
+#endif
+}
+
 __global__ void __launch_bounds__(256)
 relayout_kernel(const float* __restrict__ src, float* __restrict__ dst, int nx, int ny, int nz,
-                int TX, int TY) {
+                int TX, int TY, unsigned* __restrict__ range_slots) {
     __shared__ __align__(16) float sm[64][72];   // row = lz*8+ly; 72-float pitch: conflict-free float4 reads
     const int tx0 = blockIdx.x * 8, ty = blockIdx.y, tz = blockIdx.z;
     const int t = threadIdx.x;
     const int xo = t & 63;
     const int xs = min(tx0 * 8 + xo, nx - 1);
+    float vmin = INFINITY, vmax = -INFINITY;
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
         const int row = (t >> 6) + 4 * k;
         const int z = min(tz * 8 + (row >> 3), nz - 1);
         const int y = min(ty * 8 + (row & 7), ny - 1);
-        sm[row][xo] = __ldcs(src + ((size_t)z * ny + y) * nx + xs);
+        const float val = __ldcs(src + ((size_t)z * ny + y) * nx + xs);
+        sm[row][xo] = val;
+        vmin = fminf(vmin, val);      // fminf/fmaxf ignore NaN (blanked voxels)
+        vmax = fmaxf(vmax, val);
     }
+    // min/max of the cube, fused into the one pass that reads it (each GPU computes the
+    // minimum and maximum of its portion).  Order-preserving unsigned keys, RANGE_SLOTS slot pairs to keep the
+    // atomics uncontended; the host reduces the slots.
+    for (int sft = 16; sft > 0; sft >>= 1) {
+        vmin = fminf(vmin, __shfl_xor_sync(0xffffffffu, vmin, sft));
+        vmax = fmaxf(vmax, __shfl_xor_sync(0xffffffffu, vmax, sft));
+    }
+    __shared__ float s_min[8], s_max[8];
+    if ((t & 31) == 0) { s_min[t >> 5] = vmin; s_max[t >> 5] = vmax; }
     __syncthreads();
+    if (t == 0 && range_slots) {      // one candidate per CTA; the atomic is issued only if it would change the slot
+        float lo = s_min[0], hi = s_max[0];
+#pragma unroll
+        for (int w = 1; w < 8; ++w) { lo = fminf(lo, s_min[w]); hi = fmaxf(hi, s_max[w]); }
+        if (lo <= hi) {               // false only if every voxel seen was NaN
+            unsigned* slot = range_slots + 2 * ((blockIdx.x + 7u * blockIdx.y + 13u * blockIdx.z) & (RANGE_SLOTS - 1));
+            const unsigned klo = float_key(lo), khi = float_key(hi);
+            if (klo < *(volatile unsigned*)slot) atomicMin(slot, klo);
+            if (khi > *(volatile unsigned*)(slot + 1)) atomicMax(slot + 1, khi);
+        }
+    }
     const int ntile = min(8, TX - tx0);
     float4* out = reinterpret_cast<float4*>(dst + ((size_t)((size_t)tz * TY + ty) * TX + tx0) * TILE_ELEMS);
 #pragma unroll
@@ -235,15 +289,14 @@ __device__ __forceinline__ void classify_blend(const float4* __restrict__ tf, co
 // INSTR = 1 is the measuring build (samples evaluated, sector bitmap), never the product path.
 // ------------------------------------------------------------------------------------------------
 template <int MODE, int INSTR>
-__global__ void __launch_bounds__(CTA_THREADS)
+__global__ void __launch_bounds__(CTA_THREADS, VR_CAST_MINBLOCKS)
 cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ bricks, int n_bricks,
             const float* __restrict__ vol, const float4* __restrict__ tf_global, float* __restrict__ img,
             unsigned long long* __restrict__ counters, unsigned* __restrict__ bitmap) {
     __shared__ __align__(16) float4 tf[MODE == MODE_EA ? 512 : 1];
     __shared__ int s_brick;
     if (MODE == MODE_EA) {
-        tf[threadIdx.x] = tf_global[threadIdx.x];
-        tf[threadIdx.x + 256] = tf_global[threadIdx.x + 256];
+        for (int i = threadIdx.x; i < 512; i += CTA_THREADS) tf[i] = tf_global[i];
     }
     if (threadIdx.x == 0) {               // which brick owns this CTA: last brick with tile0 <= blockIdx.x
         int lo = 0, hi = n_bricks - 1;
@@ -259,8 +312,8 @@ cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ 
     const int tiles_x = br->tiles_x;
     const int tyi = tloc / tiles_x, txi = tloc - tyi * tiles_x;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int lx = txi * CTA_PX + (warp & 1) * 8 + (lane & 7);
-    const int ly = tyi * CTA_PX + (warp >> 1) * 4 + (lane >> 3);
+    const int lx = txi * CTA_W + (warp & 1) * 8 + (lane & 7);
+    const int ly = tyi * CTA_H + (warp >> 1) * 4 + (lane >> 3);
     if (lx >= br->rw || ly >= br->rh) return;
     const int px = br->rx0 + lx, py = br->ry0 + ly;
 
@@ -329,17 +382,16 @@ cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ 
         // Row-cached sampler (sampler.cuh); the blend of sample j-1 is issued after the loads of sample j
         // so that classification and blending overlap the load latency.
         RowCache K;
-        K.have = false; K.prev_straddle = false; K.cx = 0; K.iy = 0; K.iz = 0;
-        K.e[0][0] = K.e[0][1] = K.e[1][0] = K.e[1][1] = 0.0f;
-        K.r[0][0] = K.r[0][1] = K.r[1][0] = K.r[1][1] = make_float4(0.f, 0.f, 0.f, 0.f);
-        const bool ypos = dsy >= 0.0, zpos = dsz >= 0.0;
-        float vprev = sample_cached(vol, P.ty_stride, P.slab_stride, nxm1, nym1, nzm1, q0x, q0y, q0z, ypos, zpos, K);
+        cache_init(K);
+        const unsigned long long vol_base = reinterpret_cast<unsigned long long>(vol);
+        const unsigned slab_bytes = P.slab_stride * 4u;
+        float vprev = sample_cached(vol_base, P.ty_stride, slab_bytes, nxm1, nym1, nzm1, q0x, q0y, q0z, K);
         bool done = false;
         for (int j = 1; j < n; ++j) {
             const float jf = (float)j;
-            const float v = sample_cached(vol, P.ty_stride, P.slab_stride, nxm1, nym1, nzm1,
+            const float v = sample_cached(vol_base, P.ty_stride, slab_bytes, nxm1, nym1, nzm1,
                                           fmaf(jf, hx, fmaf(jf, ex, q0x)), fmaf(jf, hy, fmaf(jf, ey, q0y)),
-                                          fmaf(jf, hz, fmaf(jf, ez, q0z)), ypos, zpos, K);
+                                          fmaf(jf, hz, fmaf(jf, ez, q0z)), K);
             if (MODE == MODE_EA) {
                 classify_blend(tf, P, vprev, Cr, Cg, Cb, A);
                 if (P.ert_on && A >= P.ert) { done = true; break; }

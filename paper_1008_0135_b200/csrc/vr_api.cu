@@ -41,6 +41,9 @@ struct vr_volume {
     float* d_tiled = nullptr;
     cudaStream_t stream = nullptr;
     float relayout_ms = 0.f;
+    unsigned* d_range = nullptr;      // RANGE_SLOTS x (min key, max key), written by the re-layout pass
+    float data_min = 0.f, data_max = 0.f;
+    bool has_range = false;
 
     bool has_tf = false;
     float tf_host[1024];
@@ -122,8 +125,8 @@ void build_frame(const vr_volume* vol, const vr_camera* cam, int W, int H, float
         for (int a = 0; a < 3; ++a) { r.lo[a] = bp.lo[a]; r.hi[a] = bp.hi[a]; }
         r.rx0 = bp.rx0; r.ry0 = bp.ry0; r.rw = bp.rw; r.rh = bp.rh;
         r.tile0 = tiles;
-        r.tiles_x = (bp.rw + vr::CTA_PX - 1) / vr::CTA_PX;
-        const int tiles_y = (bp.rh + vr::CTA_PX - 1) / vr::CTA_PX;
+        r.tiles_x = (bp.rw + vr::CTA_W - 1) / vr::CTA_W;
+        const int tiles_y = (bp.rh + vr::CTA_H - 1) / vr::CTA_H;
         tiles += r.tiles_x * tiles_y;
         if (cropped && !direct) {
             r.img_base = (long long)pool; r.img_stride = bp.rw; r.ox = bp.rx0; r.oy = bp.ry0;
@@ -226,12 +229,13 @@ vr_status vr_create_volume(const int dims[3], const float* d_data, vr_volume** o
     if (!v) return fail(VR_ERR_OOM, "vr_create_volume: host allocation failed");
     for (int a = 0; a < 3; ++a) v->dims[a] = dims[a];
     v->TX = (dims[0] + 1 + 7) / 8; v->TY = (dims[1] + 1 + 7) / 8; v->TZ = (dims[2] + 1 + 7) / 8;
-    if ((double)v->TX * v->TY * vr::TILE_ELEMS >= 4294967296.0) {
+    if ((double)v->TX * v->TY * vr::TILE_ELEMS >= 1073741824.0) {   // slab bytes and in-slab offsets stay 32-bit
         delete v;
         return fail(VR_ERR_INVALID_ARG, "vr_create_volume: nx*ny too large for 32-bit in-slab offsets");
     }
     v->tiled_elems = (size_t)v->TX * v->TY * v->TZ * vr::TILE_ELEMS;
     cudaError_t e = cudaMalloc(&v->d_tiled, v->tiled_elems * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc(&v->d_range, 2 * vr::RANGE_SLOTS * sizeof(unsigned));
     if (e == cudaSuccess) e = cudaMalloc(&v->d_tf_ea, 512 * sizeof(float4));
     if (e == cudaSuccess) e = cudaMalloc(&v->d_tf_raw, 256 * sizeof(float4));
     if (e == cudaSuccess) e = cudaMalloc(&v->d_bricks, VR_MAX_BRICKS * sizeof(vr::BrickRec));
@@ -242,12 +246,27 @@ vr_status vr_create_volume(const int dims[3], const float* d_data, vr_volume** o
     for (int k = 0; k < 4 && e == cudaSuccess; ++k) e = cudaEventCreate(&v->ev[k]);
     if (e == cudaSuccess) {
         dim3 grid((v->TX + 7) / 8, v->TY, v->TZ);
+        std::vector<unsigned> init(2 * vr::RANGE_SLOTS);
+        for (int k = 0; k < vr::RANGE_SLOTS; ++k) { init[2 * k] = 0xffffffffu; init[2 * k + 1] = 0u; }
+        cudaMemcpyAsync(v->d_range, init.data(), init.size() * sizeof(unsigned), cudaMemcpyHostToDevice, v->stream);
         cudaEventRecord(e0, v->stream);
-        vr::relayout_kernel<<<grid, 256, 0, v->stream>>>(d_data, v->d_tiled, dims[0], dims[1], dims[2], v->TX, v->TY);
+        vr::relayout_kernel<<<grid, 256, 0, v->stream>>>(d_data, v->d_tiled, dims[0], dims[1], dims[2], v->TX, v->TY,
+                                                         v->d_range);
         cudaEventRecord(e1, v->stream);
         e = cudaGetLastError();
         if (e == cudaSuccess) e = cudaStreamSynchronize(v->stream);
         if (e == cudaSuccess) cudaEventElapsedTime(&v->relayout_ms, e0, e1);
+        if (e == cudaSuccess) {
+            std::vector<unsigned> slots(2 * vr::RANGE_SLOTS);
+            e = cudaMemcpy(slots.data(), v->d_range, slots.size() * sizeof(unsigned), cudaMemcpyDeviceToHost);
+            unsigned kmin = 0xffffffffu, kmax = 0u;
+            for (int k = 0; k < vr::RANGE_SLOTS; ++k) {
+                kmin = std::min(kmin, slots[2 * k]); kmax = std::max(kmax, slots[2 * k + 1]);
+            }
+            if (kmin <= kmax) {
+                v->data_min = vr::key_float(kmin); v->data_max = vr::key_float(kmax); v->has_range = true;
+            }
+        }
     }
     if (e0) cudaEventDestroy(e0);
     if (e1) cudaEventDestroy(e1);
@@ -263,6 +282,7 @@ vr_status vr_create_volume(const int dims[3], const float* d_data, vr_volume** o
 void vr_destroy_volume(vr_volume* v) {
     if (!v) return;
     if (v->d_tiled) cudaFree(v->d_tiled);
+    if (v->d_range) cudaFree(v->d_range);
     if (v->d_tf_ea) cudaFree(v->d_tf_ea);
     if (v->d_tf_raw) cudaFree(v->d_tf_raw);
     if (v->d_bricks) cudaFree(v->d_bricks);
@@ -451,6 +471,14 @@ vr_status vr_volume_info(const vr_volume* vol, float* h_relayout_ms, long long* 
     if (!vol) return fail(VR_ERR_INVALID_ARG, "vr_volume_info: volume is NULL");
     if (h_relayout_ms) *h_relayout_ms = vol->relayout_ms;
     if (h_tiled_bytes) *h_tiled_bytes = (long long)(vol->tiled_elems * sizeof(float));
+    return VR_OK;
+}
+
+vr_status vr_volume_range(const vr_volume* vol, float* h_min, float* h_max) {
+    if (!vol) return fail(VR_ERR_INVALID_ARG, "vr_volume_range: volume is NULL");
+    if (!vol->has_range) return fail(VR_ERR_STATE, "vr_volume_range: the cube holds no finite-ordered value (all NaN)");
+    if (h_min) *h_min = vol->data_min;
+    if (h_max) *h_max = vol->data_max;
     return VR_OK;
 }
 

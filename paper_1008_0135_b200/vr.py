@@ -19,7 +19,7 @@ VR_MAX_BRICKS = 512
 
 SYMBOLS = ["vr_create_volume", "vr_destroy_volume", "vr_set_stream", "vr_set_transfer_function",
            "vr_set_bricks", "vr_render", "vr_render_to_host", "vr_render_bricks", "vr_composite",
-           "vr_plan_bricks", "vr_measure", "vr_get_stage_ms", "vr_volume_info", "vr_export_linear", "vr_last_error"]
+           "vr_plan_bricks", "vr_measure", "vr_get_stage_ms", "vr_volume_info", "vr_volume_range", "vr_export_linear", "vr_last_error"]
 
 
 class vr_camera(C.Structure):
@@ -61,6 +61,7 @@ def lib():
                                  C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
         L.vr_get_stage_ms.argtypes = [vp, fp, fp]
         L.vr_volume_info.argtypes = [vp, fp, C.POINTER(C.c_longlong)]
+        L.vr_volume_range.argtypes = [vp, fp, fp]
         L.vr_export_linear.argtypes = [vp, vp]
         L.vr_last_error.argtypes = []
         L.vr_last_error.restype = C.c_char_p
@@ -208,6 +209,12 @@ class Volume:
         ms, nb = C.c_float(0), C.c_longlong(0)
         _check(lib().vr_volume_info(self._h, C.byref(ms), C.byref(nb)))
         return ms.value, nb.value
+
+    def vr_volume_range(self):
+        """(min, max) of the cube, NaN ignored, from the re-layout pass."""
+        a, b = C.c_float(0), C.c_float(0)
+        _check(lib().vr_volume_range(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
 
     def vr_export_linear(self):
         import torch

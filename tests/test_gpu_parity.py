@@ -271,3 +271,25 @@ def test_measure_counts_every_sample_once(vr, oracle):
         assert samples == ref["samples"]
         total_sectors = -(-71 // 8) * -(-46 // 8) * -(-53 // 8) * 64
         assert 0 < sectors <= total_sectors
+
+
+def test_volume_range_equals_library_min_max(vr):
+    """NEXT-1: min/max fused into the re-layout pass = torch.min/max, bit-exact; NaN ignored."""
+    import torch
+    for dims, seed in [((61, 35, 19), 1), ((64, 64, 64), 2), ((1, 1, 1), 3), ((200, 9, 3), 4), ((130, 70, 33), 5)]:
+        g = torch.Generator(device="cuda").manual_seed(seed)
+        cube = torch.randn((dims[2], dims[1], dims[0]), generator=g, device="cuda") * 7.0 - 2.0
+        vol = vr.Volume(cube)
+        lo, hi = vol.vr_volume_range()
+        vol.close()
+        assert lo == cube.min().item() and hi == cube.max().item(), dims
+    cube = torch.full((9, 10, 11), -5.0, device="cuda")
+    cube[3, 4, 5] = float("nan"); cube[0, 0, 0] = -9.5; cube[8, 9, 10] = -0.25
+    vol = vr.Volume(cube)
+    assert vol.vr_volume_range() == (-9.5, -0.25)
+    vol.close()
+    vol = vr.Volume(torch.full((4, 4, 4), float("nan"), device="cuda"))
+    with pytest.raises(vr.VrError) as e:
+        vol.vr_volume_range()
+    assert e.value.status == vr.VR_ERR_STATE
+    vol.close()
