@@ -340,6 +340,54 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+# ------------------------------------------------------------------------------------------------
+def run_sweep(args):
+    """BASELINE.json configs[4]: MIP point + EA sweep (bricks 1/8/64 x step 1/4,1/2,1 x image 512/1024/2048) on
+    config 3's cube, orthographic az 30 el 20, early termination off.  One JSON line per point (1 GPU)."""
+    from paper_1008_0135_b200 import vr
+    vr.lib()
+    torch.cuda.set_device(0)
+    w = wl.config(3)
+    cube = w.cube("cuda")
+    torch.cuda.synchronize()
+    vol = vr.Volume(cube)
+    vol.vr_set_transfer_function(w.table, w.vmin, w.vmax)
+    cs = wl.orbit_camera(w.dims, 30.0, 20.0, wl.PROJ_ORTHO)
+    cam = vr.camera_from_spec(cs)
+    peak, peak_src = measured_peak_gbs()
+    reps = max(3, min(args.steps, 10))
+    for pt in wl.sweep_points():
+        size, step, mode, bricks = pt["size"], pt["step"], pt["mode"], pt["bricks"]
+        vol.vr_set_bricks(*bricks)
+        out = torch.empty((size, size, 4), dtype=torch.float32, device="cuda")
+        for _ in range(3):
+            vol.vr_render(cam, size, size, step, mode, 0.0, out=out)
+        torch.cuda.synchronize()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * reps)]
+        cast = []
+        for k in range(reps):
+            ev[2 * k].record()
+            vol.vr_render(cam, size, size, step, mode, 0.0, out=out)
+            ev[2 * k + 1].record()
+            cast.append(vol.vr_get_stage_ms()[0])
+        torch.cuda.synchronize()
+        ms = sorted(ev[2 * k].elapsed_time(ev[2 * k + 1]) for k in range(reps))
+        samples, sectors = vol.vr_measure(cam, size, size, step, mode, 0.0)
+        best, med = ms[0], ms[len(ms) // 2]
+        cast_med = sorted(cast)[len(cast) // 2]
+        B = bricks[0] * bricks[1] * bricks[2]
+        print(json.dumps({"sweep_point": {"mode": "MIP" if mode else "EA", "bricks": B, "step_voxels": step,
+                                          "image": f"{size}x{size}"},
+                          "ms_per_frame_best": best, "ms_per_frame_median": med, "cast_ms_median": cast_med,
+                          "samples": samples, "gsamples_per_s": samples / (med * 1e-3) / 1e9,
+                          "algorithmic_GB": 32e-9 * sectors, "bytes_per_sample": 32.0 * sectors / samples,
+                          "hbm_GBps_algorithmic": 32e-9 * sectors / (cast_med * 1e-3),
+                          "frac_of_peak": 32e-9 * sectors / (cast_med * 1e-3) / peak, "peak": peak,
+                          "side_of_ridge": "hbm" if 32.0 * sectors / samples > 14.0 else "alu/lsu"}), flush=True)
+        del out
+    vol.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -351,11 +399,14 @@ def main():
                     help="oracle legs render every n-th pixel in x and y (default 1 = the full frame for cpu_baseline, 4 for --impl reference)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--stage-times", action="store_true", help=argparse.SUPPRESS)
+    ap.add_argument("--sweep", action="store_true", help="run BASELINE.json configs[4] (28 points) instead of the headline")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.cpu_stride is None:
         args.cpu_stride = 4 if args.impl == "reference" else 1
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
