@@ -109,6 +109,11 @@ void build_frame(const vr_volume* vol, const vr_camera* cam, int W, int H, float
     P.inv_range = 1.0f / (vol->vmax - vol->vmin);
     P.ert_on = (ert > 0.0f && ert < 1.0f) ? 1 : 0;
     P.ert = ert;
+    {   // first table entry with alpha > 0 (the per-step correction keeps zeros zero)
+        int j0 = 0;
+        while (j0 < 256 && !(vol->tf_host[4 * j0 + 3] > 0.0f)) ++j0;
+        P.x_zero_below = (float)(j0 - 1);
+    }
 
     std::vector<vr::BrickPlan> plan;
     vr::plan_bricks(vol->dims, vol->bricks, *cam, W, H, plan, f.order);
