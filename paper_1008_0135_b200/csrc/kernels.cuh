@@ -270,7 +270,7 @@ __device__ __forceinline__ float trilerp(const Footprint& F) {
 #include "sampler.cuh"
 namespace vr {
 
-// O6 + O7: classify through the shared-memory table (entry m: T[m], then T[m+1]-T[m]) and blend.
+// O6 + O7: classify through the shared-memory table (256 float4 entries) and blend.
 // Transparent-sample skip: x_zero_below = (index of the first table entry with alpha > 0) - 1.  For x below it both
 // entries the lookup would blend have alpha exactly 0, so the sample adds exactly nothing to C and A (as in
 // the oracle) and the table reads and the blend are skipped — with a noise-suppressing table
@@ -282,7 +282,8 @@ __device__ __forceinline__ void classify_blend(const float4* __restrict__ tf, co
     const float r = fminf(__fadd_rd(x, 8388608.0f), 8388608.0f + 254.0f);   // 2^23 + min(floor(x),254)
     const unsigned m = __float_as_uint(r) & 0xffu;
     const float w = x - (r - 8388608.0f);
-    const float4 t0 = tf[2 * m], dt = tf[2 * m + 1];
+    const float4 t0 = tf[m], t1 = tf[m + 1];
+    const float4 dt = make_float4(t1.x - t0.x, t1.y - t0.y, t1.z - t0.z, t1.w - t0.w);
     float a = fmaf(w, dt.w, t0.w);
     a = (value == value) ? a : 0.0f;                                         // O5/A14: NaN sample skipped
     const float wgt = (1.0f - A) * a;
@@ -302,10 +303,10 @@ __global__ void __launch_bounds__(CTA_THREADS, VR_CAST_MINBLOCKS)
 cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ bricks, int n_bricks,
             const float* __restrict__ vol, const float4* __restrict__ tf_global, float* __restrict__ img,
             unsigned long long* __restrict__ counters, unsigned* __restrict__ bitmap) {
-    __shared__ __align__(16) float4 tf[MODE == MODE_EA ? 512 : 1];
+        __shared__ __align__(16) float4 tf[MODE == MODE_EA ? 256 : 1];   // 4 KB: keeps the L1 share of the SM large
     __shared__ int s_brick;
     if (MODE == MODE_EA) {
-        for (int i = threadIdx.x; i < 512; i += CTA_THREADS) tf[i] = tf_global[i];
+        for (int i = threadIdx.x; i < 256; i += CTA_THREADS) tf[i] = tf_global[i];
     }
     if (threadIdx.x == 0) {               // which brick owns this CTA: last brick with tile0 <= blockIdx.x
         int lo = 0, hi = n_bricks - 1;

@@ -49,7 +49,7 @@ struct vr_volume {
     float tf_host[1024];
     float vmin = 0.f, vmax = 1.f;
     double tf_step = -1.0;            // step the device EA table is currently corrected for
-    float4* d_tf_ea = nullptr;        // 512 float4: T_step[m], T_step[m+1]-T_step[m]
+    float4* d_tf_ea = nullptr;        // 256 float4: the table corrected for the current step (O6)
     float4* d_tf_raw = nullptr;       // 256 float4: table as given (MIP colour, O8)
 
     int bricks[3] = {1, 1, 1};
@@ -160,7 +160,7 @@ vr_status upload_plan(vr_volume* vol, Frame& f) {
     return VR_OK;
 }
 
-// O6: per-entry opacity correction for this step, in double, then the (T, dT) pairs the caster reads.
+// O6: per-entry opacity correction for this step, in double.
 vr_status upload_tf_for_step(vr_volume* vol, double step) {
     if (vol->tf_step == step) return VR_OK;
     std::vector<float> t(256 * 4);
@@ -169,13 +169,7 @@ vr_status upload_tf_for_step(vr_volume* vol, double step) {
         const double a = (double)vol->tf_host[4 * j + 3];
         t[4 * j + 3] = (float)((step == 1.0) ? a : 1.0 - std::pow(1.0 - a, step));
     }
-    std::vector<float> pairs(512 * 4, 0.0f);
-    for (int m = 0; m < 256; ++m)
-        for (int c = 0; c < 4; ++c) {
-            pairs[8 * m + c] = t[4 * m + c];
-            pairs[8 * m + 4 + c] = (m < 255) ? (float)((double)t[4 * (m + 1) + c] - (double)t[4 * m + c]) : 0.0f;
-        }
-    VR_CUDA(cudaMemcpyAsync(vol->d_tf_ea, pairs.data(), sizeof(float) * 2048, cudaMemcpyHostToDevice, vol->stream),
+    VR_CUDA(cudaMemcpyAsync(vol->d_tf_ea, t.data(), sizeof(float) * 1024, cudaMemcpyHostToDevice, vol->stream),
             "upload transfer function");
     vol->tf_step = step;
     return VR_OK;
