@@ -36,8 +36,8 @@ from paper_1008_0135_b200 import workloads as wl
 METRIC = "ms_per_frame_1024x1024"
 UNIT = "ms/frame"
 # Per-launch DRAM traffic of cast_kernel<EA> from the committed `ncu --set full` capture
-# (dram__bytes_read.sum + dram__bytes_write.sum, mean of the two launches in profiles/r01c_cast_full.md).
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 27.46e9
+# (dram__bytes_read.sum + dram__bytes_write.sum, mean of the two r01d launches in profiles/r01cd_cast_full.md).
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 27.19e9
 
 
 def env_int(name, default):

@@ -28,7 +28,10 @@ constexpr int TILE_ELEMS = 512;         // 8^3 floats = 2 KB, x-rows of 32 B = o
 #ifndef VR_CAST_MINBLOCKS
 #define VR_CAST_MINBLOCKS 7
 #endif
-constexpr int CTA_W = 16;               // a CTA renders a CTA_W x CTA_H pixel tile: warps of 8x4 pixels, 2 across
+#ifndef VR_CTA_W
+#define VR_CTA_W 16
+#endif
+constexpr int CTA_W = VR_CTA_W;               // a CTA renders a CTA_W x CTA_H pixel tile: warps of 8x4 pixels, 2 across
 constexpr int CTA_H = VR_CTA_H;
 constexpr int CTA_THREADS = CTA_W * CTA_H;
 constexpr int MODE_EA = 0, MODE_MIP = 1;
