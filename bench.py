@@ -110,7 +110,9 @@ class ClockSampler:
 
 def workload_for(args):
     w = wl.config(args.config)
-    views = wl.orbit_azimuths() if args.config == 3 else [w.az_deg]
+    if getattr(args, "image", None):
+        w.W = w.H = int(args.image)
+    views = wl.orbit_azimuths() if args.config in (3, 5) else [w.az_deg]   # 5: rotation about y at el 0 (Fig 7)
     return w, views
 
 
@@ -394,9 +396,10 @@ def main():
     ap.add_argument("--steps", type=int, default=36)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (0..3); 3 is the headline")
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (0..3), 3 is the headline; 5 = N-body-like 1024^3 cube")
     ap.add_argument("--cpu-stride", type=int, default=None,
                     help="oracle legs render every n-th pixel in x and y (default 1 = the full frame for cpu_baseline, 4 for --impl reference)")
+    ap.add_argument("--image", type=int, default=None, help="override the image size (W = H), e.g. 512 for Fig 12's comparison")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--stage-times", action="store_true", help=argparse.SUPPRESS)
     ap.add_argument("--sweep", action="store_true", help="run BASELINE.json configs[4] (28 points) instead of the headline")

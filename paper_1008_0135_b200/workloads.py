@@ -238,6 +238,43 @@ def cube_gass_like(dims, seed, device="cpu", n_sources=10000, field_amp=20.0, ch
     return cube
 
 
+def cube_nbody_like(dims, seed, device="cpu", sigma=1.6, coarse=2):
+    """Second workload (the paper's third dataset, an N-body density cube of 1024^3,
+    Table 3): a log-normal density field rho = exp(sigma*g - sigma^2/2), g a unit-rms Gaussian random
+    field with P(k) ~ k^-2 generated at 1/coarse resolution by FFT and trilinearly upsampled (smooth at the voxel
+    scale, like a CIC-binned simulation), plus 2 % multiplicative white noise.  Positive, mean ~1, filaments and
+    knots reaching ~50."""
+    nx, ny, nz = dims
+    g = _gen(seed, device)
+    q = int(coarse)
+    cz, cy, cx = max(2, -(-nz // q)), max(2, -(-ny // q)), max(2, -(-nx // q))
+    white = torch.randn((cz, cy, cx), generator=g, device=device, dtype=torch.float32)
+    kz = torch.fft.fftfreq(cz, device=device)[:, None, None]
+    ky = torch.fft.fftfreq(cy, device=device)[None, :, None]
+    kx = torch.fft.rfftfreq(cx, device=device)[None, None, :]
+    k = torch.sqrt(kz * kz + ky * ky + kx * kx)
+    k[0, 0, 0] = 1.0
+    amp = k ** (-1.0)
+    amp[0, 0, 0] = 0.0
+    field = torch.fft.irfftn(torch.fft.rfftn(white) * amp, s=(cz, cy, cx))
+    del white, k, amp
+    field = field / field.std()
+    cube = torch.empty((nz, ny, nx), dtype=torch.float32, device=device)
+    chunk = max(1, (1 << 27) // (nx * ny))
+    for s0 in range(0, nz, chunk):
+        s1 = min(nz, s0 + chunk)
+        zc = ((torch.arange(s0, s1, device=device, dtype=torch.float32) + 0.5) / q - 0.5).clamp(0, cz - 1)
+        i0 = zc.floor().long()
+        i1 = (i0 + 1).clamp(max=cz - 1)
+        fz = (zc - i0.float())[:, None, None]
+        slab = field[i0] * (1 - fz) + field[i1] * fz
+        up = torch.nn.functional.interpolate(slab[None], size=(ny, nx), mode="bilinear", align_corners=False)[0]
+        noise = torch.empty_like(up).normal_(0.0, 0.02, generator=g)
+        cube[s0:s1] = torch.exp(sigma * up - 0.5 * sigma * sigma) * (1.0 + noise)
+        del slab, up, noise
+    return cube
+
+
 # ------------------------------------------------------------------ configs -------------------
 @dataclass
 class Workload:
@@ -273,9 +310,9 @@ class Workload:
         kw = dict(self.cube_kwargs)
         vol = (dims[0] * dims[1] * dims[2]) / (self.dims[0] * self.dims[1] * self.dims[2])
         key, base = {"cube_blobs": ("n_blobs", 4), "cube_blobs_band": ("n_blobs", 200),
-                     "cube_hipass_like": ("n_sources", 5000),
-                     "cube_gass_like": ("n_sources", 10000)}[self.cube_fn]
-        if self.cube_fn != "cube_blobs":
+                     "cube_hipass_like": ("n_sources", 5000), "cube_gass_like": ("n_sources", 10000),
+                     "cube_nbody_like": (None, 0)}[self.cube_fn]
+        if key is not None and self.cube_fn != "cube_blobs":
             kw[key] = max(1, int(round(kw.get(key, base) * vol)))
         return Workload(self.name + f"_x{factor:g}", dims, self.seed, self.cube_fn, self.bricks,
                         W or self.W, H or self.H, self.projection, self.az_deg, self.el_deg,
@@ -284,7 +321,7 @@ class Workload:
 
 def config(i):
     """BASELINE.json `configs[i]` (i = 0..3; config 4 is a sweep over config 3's cube, see
-    sweep_points()).  Items BASELINE.json leaves open are fixed as DESIGN.md "Inputs" says."""
+    sweep_points(); 5 is the extra N-body-like workload).  Items BASELINE.json leaves open are fixed as DESIGN.md "Inputs" says."""
     if i == 0:
         return Workload("cfg0_64cube", (64, 64, 64), 0, "cube_blobs", (1, 1, 1), 256, 256,
                         PROJ_ORTHO, 30.0, 20.0, 0.5, MODE_EA, 0.0, tf_ramp(0.1), -3.0, 8.0)
@@ -301,7 +338,13 @@ def config(i):
         return Workload("cfg3_gass_2048x2048x1600", (2048, 2048, 1600), 3, "cube_gass_like",
                         (2, 2, 2), 1024, 1024, PROJ_PERSP, 30.0, 20.0, 1.0, MODE_EA, 0.995, tab,
                         -3.0, 30.0)
-    raise ValueError("config index must be 0..3")
+    if i == 5:
+        # not a BASELINE.json config: the paper's N-body cube (Table 3) with the rotation-about-y protocol of
+        # Figs 7 and 12: el = 0, orthographic, early termination off
+        tab = tf_piecewise(0.0, 20.0, [(1.0, 0.0), (4.0, 0.05), (20.0, 0.4)])
+        return Workload("cfg5_nbody_1024cube", (1024, 1024, 1024), 5, "cube_nbody_like", (2, 2, 2), 1024, 1024,
+                        PROJ_ORTHO, 30.0, 0.0, 1.0, MODE_EA, 0.0, tab, 0.0, 20.0)
+    raise ValueError("config index must be 0..3 or 5")
 
 
 def orbit_azimuths():

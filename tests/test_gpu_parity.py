@@ -87,9 +87,10 @@ def test_config1_bricks_perspective_ert(vr, oracle):
     assert ref_off[..., 3].max() > 0.5
 
 
-@pytest.mark.parametrize("cfg,factor,size", [(2, 1.0 / 8, 256), (3, 1.0 / 8, 256)])
+@pytest.mark.parametrize("cfg,factor,size", [(2, 1.0 / 8, 256), (3, 1.0 / 8, 256), (5, 1.0 / 8, 256)])
 def test_scaled_headline_configs(vr, oracle, cfg, factor, size):
-    """Configs 2 and 3 (HIPASS-/GASS-shaped) at 1/8 linear size: same recipe, bricks, camera, table."""
+    """Configs 2, 3 (HIPASS-/GASS-shaped) and the N-body-like workload at 1/8 linear size: same recipe, bricks,
+    camera, table."""
     w = wl.config(cfg).scaled(factor, W=size, H=size)
     cube = w.cube("cuda")
     host = cube.cpu().numpy()
