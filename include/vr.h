@@ -79,6 +79,13 @@ vr_status vr_set_transfer_function(vr_volume* vol, const float rgba[256 * 4], fl
  *     DESIGN.md O9/A10).  Default 1,1,1.  INVALID_ARG: b_a < 1, b_a > n_a, product > VR_MAX_BRICKS. */
 vr_status vr_set_bricks(vr_volume* vol, int bx, int by, int bz);
 
+/* Sub-cube / spectral-channel selection ("a manual sub-cube"; PAPER.md:138 channels enabled or
+ *     disabled by the user): only samples inside [lo, hi) voxels are taken — e.g. lo = {0,0,z0}, hi = {nx,ny,z1}
+ *     renders channels z0..z1-1.  The sample lattice and the sampling (which still reads neighbouring voxels
+ *     across the sub-cube's faces) are unchanged: the sub-cube is one more box every brick is intersected with
+ *     (S1).  NULL, NULL restores the whole cube.  INVALID_ARG unless 0 <= lo_a <= hi_a <= n_a.       */
+vr_status vr_set_subcube(vr_volume* vol, const int lo[3], const int hi[3]);
+
 /* a1-a7  One frame: per-brick ray casting inside each brick's rendering rectangle
  *     (PAPER.md:150), then depth-ordered composition into d_out_rgba.
  *     step_voxels: sampling distance along the ray in voxels, > 0.

@@ -187,6 +187,22 @@ static void brick_box(const int dims[3], const int bricks[3], const int idx[3], 
     }
 }
 
+/* O9 for an explicit box [lo,hi] (voxel units): owned range of the global lattice. */
+static int box_span(const double o[3], const double d[3], const double lo[3], const double hi[3], double step,
+                    double t_near, double t_far, double* t_in, long long* i_lo, long long* i_hi) {
+    double t0, t1;
+    *t_in = 0.0; *i_lo = 0; *i_hi = 0;
+    for (int a = 0; a < 3; ++a) if (!(hi[a] > lo[a])) return 0;
+    if (!vro_slab(o, d, lo, hi, &t0, &t1)) return 0;
+    if (t0 < t_near) t0 = t_near;
+    if (t1 > t_far) t1 = t_far;
+    if (!(t1 > t0)) return 0;
+    *t_in = t0;
+    *i_lo = lattice_index(t0, t_near, step);
+    *i_hi = lattice_index(t1, t_near, step);
+    return *i_hi > *i_lo;
+}
+
 int vro_brick_span(const double o[3], const double d[3], const int dims[3], const int bricks[3],
                    int bi, int bj, int bk, double step, double t_near, double t_far,
                    double* t_in, long long* i_lo, long long* i_hi) {
@@ -253,12 +269,22 @@ static int cmp_key(const void* x, const void* y) {
 }
 
 /* ---------------------------------------------------------------- O1-O11 pixels ----------- */
-int vro_render_pixels(const float* data, const int dims[3], const float rgba[1024], float vmin_f,
-                      float vmax_f, const int bricks_in[3], const vro_camera* cam, int W, int H,
-                      float step_f, int mode, float ert_f, int route, long long n_pix,
-                      const int* px, const int* py, float* out_rgba, float* out_scalar,
-                      float* out_brick, long long* out_samples, int threads) {
+int vro_render_pixels_sub(const float* data, const int dims[3], const float rgba[1024], float vmin_f,
+                          float vmax_f, const int bricks_in[3], const int sub_lo[3], const int sub_hi[3],
+                          const vro_camera* cam, int W, int H, float step_f, int mode, float ert_f, int route,
+                          long long n_pix, const int* px, const int* py, float* out_rgba, float* out_scalar,
+                          float* out_brick, long long* out_samples, int threads) {
     if (!data || !dims || !rgba || !cam || !out_rgba || n_pix < 0) return -1;
+    /* S1 sub-cube ("a manual sub-cube", PAPER.md:138 channel enable/disable): only samples of the
+     * global lattice that lie in [sub_lo, sub_hi) are taken; the lattice itself (O4) and the sampling (O5, whole
+     * cube) are unchanged, i.e. the sub-cube acts as one more box every brick is intersected with. */
+    int slo[3] = {0, 0, 0}, shi[3] = {dims[0], dims[1], dims[2]};
+    if (sub_lo && sub_hi)
+        for (int a = 0; a < 3; ++a) {
+            if (sub_lo[a] < 0 || sub_hi[a] > dims[a] || sub_hi[a] < sub_lo[a]) return -1;
+            slo[a] = sub_lo[a]; shi[a] = sub_hi[a];
+        }
+    const int has_sub = (sub_lo && sub_hi);
     if (dims[0] <= 0 || dims[1] <= 0 || dims[2] <= 0 || W <= 0 || H <= 0) return -1;
     if (!(step_f > 0.0f) || !(vmax_f > vmin_f)) return -1;
     if (mode != VRO_MODE_EA && mode != VRO_MODE_MIP) return -1;
@@ -291,9 +317,16 @@ int vro_render_pixels(const float* data, const int dims[3], const float rgba[102
         accum fin;
         fin.C[0] = fin.C[1] = fin.C[2] = 0.0; fin.A = 0.0; fin.M = -INFINITY;
         if (route == 0) {
-            if (n > 0)
+            long long a_lo = 0, a_hi = n;
+            if (has_sub && n > 0) {
+                double blo[3] = {(double)slo[0], (double)slo[1], (double)slo[2]};
+                double bhi[3] = {(double)shi[0], (double)shi[1], (double)shi[2]};
+                double t_in_unused;
+                if (!box_span(o, d, blo, bhi, step, t_near, t_far, &t_in_unused, &a_lo, &a_hi)) a_hi = a_lo = 0;
+            }
+            if (a_hi > a_lo)
                 total += march(data, dims, (const double(*)[4])tstep, vmin, vmax, o, d, t_near,
-                               step, 0, n, mode, ert, &fin);
+                               step, a_lo, a_hi, mode, ert, &fin);
         } else {
             brick_key keys[B > 0 ? B : 1];
             accum parts[B > 0 ? B : 1];
@@ -306,8 +339,14 @@ int vro_render_pixels(const float* data, const int dims[3], const float rgba[102
                         part->C[0] = part->C[1] = part->C[2] = 0.0;
                         part->A = 0.0; part->M = -INFINITY;
                         double t_in; long long i_lo, i_hi;
-                        if (n > 0 && vro_brick_span(o, d, dims, bricks, bi, bj, bk, step, t_near,
-                                                    t_far, &t_in, &i_lo, &i_hi)) {
+                        int idx3[3] = {bi, bj, bk};
+                        double blo[3], bhi[3];
+                        brick_box(dims, bricks, idx3, blo, bhi);
+                        for (int a = 0; a < 3; ++a) {          /* S1: brick box intersected with the sub-cube */
+                            if (blo[a] < (double)slo[a]) blo[a] = (double)slo[a];
+                            if (bhi[a] > (double)shi[a]) bhi[a] = (double)shi[a];
+                        }
+                        if (n > 0 && box_span(o, d, blo, bhi, step, t_near, t_far, &t_in, &i_lo, &i_hi)) {
                             total += march(data, dims, (const double(*)[4])tstep, vmin, vmax, o,
                                            d, t_near, step, i_lo, i_hi, mode, ert, part);
                             keys[nk].t_in = t_in; keys[nk].b = b; ++nk;
@@ -357,6 +396,14 @@ int vro_render_pixels(const float* data, const int dims[3], const float rgba[102
     free(tabs);
     if (out_samples) *out_samples = total;
     return 0;
+}
+
+int vro_render_pixels(const float* data, const int dims[3], const float rgba[1024], float vmin,
+                      float vmax, const int bricks[3], const vro_camera* cam, int W, int H, float step, int mode,
+                      float ert_alpha, int route, long long n_pix, const int* px, const int* py, float* out_rgba,
+                      float* out_scalar, float* out_brick, long long* out_samples, int threads) {
+    return vro_render_pixels_sub(data, dims, rgba, vmin, vmax, bricks, NULL, NULL, cam, W, H, step, mode, ert_alpha,
+                                 route, n_pix, px, py, out_rgba, out_scalar, out_brick, out_samples, threads);
 }
 
 int vro_render(const float* data, const int dims[3], const float rgba[1024], float vmin,

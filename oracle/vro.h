@@ -76,6 +76,15 @@ int vro_render_pixels(const float* data, const int dims[3], const float rgba[102
                       const int* px, const int* py, float* out_rgba, float* out_scalar,
                       float* out_brick, long long* out_samples, int threads);
 
+/* S1  Same with a sub-cube [sub_lo, sub_hi) in voxels (NULL, NULL = the whole cube): only lattice samples inside
+ *     it are taken (PAPER.md:128 manual sub-cube; PAPER.md:138 spectral channels enabled/disabled = a z range);
+ *     lattice (O4) and sampling (O5) are unchanged, every brick box is intersected with the sub-cube.            */
+int vro_render_pixels_sub(const float* data, const int dims[3], const float rgba[1024], float vmin,
+                          float vmax, const int bricks[3], const int sub_lo[3], const int sub_hi[3],
+                          const vro_camera* cam, int W, int H, float step, int mode, float ert_alpha, int route,
+                          long long n_pix, const int* px, const int* py, float* out_rgba, float* out_scalar,
+                          float* out_brick, long long* out_samples, int threads);
+
 /* Full frame: every pixel, row-major [py][px].  out_brick then is [B][H][W][4] / [B][H][W].      */
 int vro_render(const float* data, const int dims[3], const float rgba[1024], float vmin,
                float vmax, const int bricks[3], const vro_camera* cam, int W, int H, float step,

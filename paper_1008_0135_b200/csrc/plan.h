@@ -76,8 +76,10 @@ inline double tan_half_fov(const vr_camera& cam) {
 inline int brick_face(int m, int n, int b) { return (int)(((long long)m * n) / b); }
 
 // a2 + a6 for every brick; order[k] = k-th brick front to back.
+// sub_lo/sub_hi (may be null): sub-cube every brick box is intersected with (S1).
 inline void plan_bricks(const int dims[3], const int bricks[3], const vr_camera& cam, int W, int H,
-                        std::vector<BrickPlan>& plan, std::vector<int>& order) {
+                        std::vector<BrickPlan>& plan, std::vector<int>& order, const int* sub_lo = nullptr,
+                        const int* sub_hi = nullptr) {
     const Basis bs = make_basis(cam);
     const bool persp = cam.projection == VR_PROJ_PERSP;
     const double asp = (double)W / (double)H;
@@ -109,6 +111,10 @@ inline void plan_bricks(const int dims[3], const int bricks[3], const vr_camera&
                 for (int a = 0; a < 3; ++a) {
                     p.lo[a] = brick_face(idx[a], dims[a], bricks[a]);
                     p.hi[a] = brick_face(idx[a] + 1, dims[a], bricks[a]);
+                    if (sub_lo && sub_hi) {            // S1: only the part of the brick inside the sub-cube
+                        p.lo[a] = std::max(p.lo[a], sub_lo[a]);
+                        p.hi[a] = std::min(p.hi[a], sub_hi[a]);
+                    }
                     if (persp) p.key += std::abs(idx[a] - eslab[a]);
                     else p.key += (bs.fwd[a] >= 0.0) ? idx[a] : bricks[a] - 1 - idx[a];
                 }
@@ -116,6 +122,10 @@ inline void plan_bricks(const int dims[3], const int bricks[3], const vr_camera&
                 // continuous pixel coordinates where pixel px covers [px, px+1).
                 double xmin = 1e300, xmax = -1e300, ymin = 1e300, ymax = -1e300;
                 bool full = false;
+                if (p.hi[0] <= p.lo[0] || p.hi[1] <= p.lo[1] || p.hi[2] <= p.lo[2]) {   // empty after S1
+                    p.rx0 = p.ry0 = p.rw = p.rh = 0;
+                    continue;
+                }
                 for (int c = 0; c < 8 && !full; ++c) {
                     double rel[3];
                     for (int a = 0; a < 3; ++a)

@@ -53,6 +53,7 @@ struct vr_volume {
     float4* d_tf_raw = nullptr;       // 256 float4: table as given (MIP colour, O8)
 
     int bricks[3] = {1, 1, 1};
+    int sub_lo[3] = {0, 0, 0}, sub_hi[3] = {0, 0, 0};   // sub-cube (S1); set to the whole cube at create
     vr::BrickRec* d_bricks = nullptr; // VR_MAX_BRICKS records
     int* d_order = nullptr;
 
@@ -116,7 +117,7 @@ void build_frame(const vr_volume* vol, const vr_camera* cam, int W, int H, float
     }
 
     std::vector<vr::BrickPlan> plan;
-    vr::plan_bricks(vol->dims, vol->bricks, *cam, W, H, plan, f.order);
+    vr::plan_bricks(vol->dims, vol->bricks, *cam, W, H, plan, f.order, vol->sub_lo, vol->sub_hi);
     const int B = (int)plan.size();
     f.recs.assign(B, vr::BrickRec());
     int tiles = 0;
@@ -226,7 +227,7 @@ vr_status vr_create_volume(const int dims[3], const float* d_data, vr_volume** o
         if (dims[a] <= 0 || dims[a] > 65528) return fail(VR_ERR_INVALID_ARG, "vr_create_volume: each dim must be in [1,65528]");
     vr_volume* v = new (std::nothrow) vr_volume();
     if (!v) return fail(VR_ERR_OOM, "vr_create_volume: host allocation failed");
-    for (int a = 0; a < 3; ++a) v->dims[a] = dims[a];
+    for (int a = 0; a < 3; ++a) { v->dims[a] = dims[a]; v->sub_hi[a] = dims[a]; }
     v->TX = (dims[0] + 1 + 7) / 8; v->TY = (dims[1] + 1 + 7) / 8; v->TZ = (dims[2] + 1 + 7) / 8;
     if ((double)v->TX * v->TY * vr::TILE_ELEMS >= 1073741824.0) {   // slab bytes and in-slab offsets stay 32-bit
         delete v;
@@ -322,6 +323,20 @@ vr_status vr_set_bricks(vr_volume* vol, int bx, int by, int bz) {
         if (b[a] < 1 || b[a] > vol->dims[a]) return fail(VR_ERR_INVALID_ARG, "vr_set_bricks: need 1 <= b_a <= n_a");
     if ((long long)bx * by * bz > VR_MAX_BRICKS) return fail(VR_ERR_INVALID_ARG, "vr_set_bricks: more than VR_MAX_BRICKS bricks");
     for (int a = 0; a < 3; ++a) vol->bricks[a] = b[a];
+    return VR_OK;
+}
+
+vr_status vr_set_subcube(vr_volume* vol, const int lo[3], const int hi[3]) {
+    if (!vol) return fail(VR_ERR_INVALID_ARG, "vr_set_subcube: volume is NULL");
+    if (!lo || !hi) {                                  // NULL, NULL: back to the whole cube
+        if (lo || hi) return fail(VR_ERR_INVALID_ARG, "vr_set_subcube: pass both corners or neither");
+        for (int a = 0; a < 3; ++a) { vol->sub_lo[a] = 0; vol->sub_hi[a] = vol->dims[a]; }
+        return VR_OK;
+    }
+    for (int a = 0; a < 3; ++a)
+        if (lo[a] < 0 || hi[a] > vol->dims[a] || hi[a] < lo[a])
+            return fail(VR_ERR_INVALID_ARG, "vr_set_subcube: need 0 <= lo_a <= hi_a <= n_a");
+    for (int a = 0; a < 3; ++a) { vol->sub_lo[a] = lo[a]; vol->sub_hi[a] = hi[a]; }
     return VR_OK;
 }
 

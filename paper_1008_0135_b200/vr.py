@@ -18,7 +18,7 @@ VR_PROJ_ORTHO, VR_PROJ_PERSP = 0, 1
 VR_MAX_BRICKS = 512
 
 SYMBOLS = ["vr_create_volume", "vr_destroy_volume", "vr_set_stream", "vr_set_transfer_function",
-           "vr_set_bricks", "vr_render", "vr_render_to_host", "vr_render_bricks", "vr_composite",
+           "vr_set_bricks", "vr_set_subcube", "vr_render", "vr_render_to_host", "vr_render_bricks", "vr_composite",
            "vr_plan_bricks", "vr_measure", "vr_get_stage_ms", "vr_volume_info", "vr_volume_range", "vr_export_linear", "vr_last_error"]
 
 
@@ -52,6 +52,7 @@ def lib():
         L.vr_set_stream.argtypes = [vp, vp]
         L.vr_set_transfer_function.argtypes = [vp, fp, C.c_float, C.c_float]
         L.vr_set_bricks.argtypes = [vp, C.c_int, C.c_int, C.c_int]
+        L.vr_set_subcube.argtypes = [vp, ip, ip]
         L.vr_render.argtypes = [vp, cam, C.c_int, C.c_int, C.c_float, C.c_int, C.c_float, vp, vp]
         L.vr_render_to_host.argtypes = [vp, cam, C.c_int, C.c_int, C.c_float, C.c_int, C.c_float, vp]
         L.vr_render_bricks.argtypes = [vp, cam, C.c_int, C.c_int, C.c_float, C.c_int, C.c_float, vp]
@@ -159,6 +160,12 @@ class Volume:
     def vr_set_bricks(self, bx, by, bz):
         _check(lib().vr_set_bricks(self._h, int(bx), int(by), int(bz)))
         self.bricks = (int(bx), int(by), int(bz))
+
+    def vr_set_subcube(self, lo=None, hi=None):
+        if lo is None and hi is None:
+            _check(lib().vr_set_subcube(self._h, None, None))
+        else:
+            _check(lib().vr_set_subcube(self._h, _i3(lo), _i3(hi)))
 
     def vr_render(self, cam, W, H, step, mode, ert_alpha=0.0, out=None, out_scalar=None):
         import torch

@@ -294,3 +294,41 @@ def test_volume_range_equals_library_min_max(vr):
         vol.vr_volume_range()
     assert e.value.status == vr.VR_ERR_STATE
     vol.close()
+
+
+def test_subcube_and_channel_range_match_oracle(vr, oracle):
+    """NEXT-3 / S1: sub-cube and spectral-channel selection, GPU vs oracle, bricked and not."""
+    import torch
+    dims = (70, 45, 52)
+    cube = wl.cube_blobs(dims, 21, "cuda", n_blobs=6, amp=6.0, sigma=5.0)
+    host = cube.cpu().numpy()
+    tab = wl.tf_ramp(0.2)
+    W, H = 120, 90
+    vol = vr.Volume(cube)
+    vol.vr_set_transfer_function(tab, -3.0, 8.0)
+    cases = [((0, 0, 10), (70, 45, 31), (1, 1, 1), wl.PROJ_ORTHO, 0),      # channels 10..30
+             ((13, 5, 7), (55, 40, 44), (2, 2, 2), wl.PROJ_PERSP, 0),      # interior box cutting every brick
+             ((0, 0, 0), (70, 45, 52), (3, 1, 2), wl.PROJ_PERSP, 0),       # whole cube
+             ((20, 0, 0), (20, 45, 52), (2, 2, 2), wl.PROJ_ORTHO, 0),      # empty
+             ((5, 9, 20), (66, 30, 40), (2, 1, 2), wl.PROJ_ORTHO, 1)]      # MIP
+    for lo, hi, bricks, proj, mode in cases:
+        cs = wl.orbit_camera(dims, 215.0, 25.0, proj)
+        vol.vr_set_bricks(*bricks)
+        vol.vr_set_subcube(lo, hi)
+        got = vol.vr_render(vr.camera_from_spec(cs), W, H, 0.5, mode, 0.0).cpu().numpy()
+        ref = oracle.render(host, tab, -3.0, 8.0, bricks, ocam(oracle, cs), W, H, 0.5, mode, 0.0, route=1,
+                            subcube=(lo, hi))["rgba"]
+        assert np.abs(got - ref).max() <= TOL_EA, (lo, hi, bricks, np.abs(got - ref).max(axis=(0, 1)))
+        if lo[0] == hi[0]:
+            assert (got == 0).all()
+    vol.vr_set_subcube()                                     # back to the whole cube
+    vol.vr_set_bricks(1, 1, 1)
+    cs = wl.orbit_camera(dims, 30.0, 20.0, wl.PROJ_ORTHO)
+    got = vol.vr_render(vr.camera_from_spec(cs), W, H, 0.5, 0, 0.0).cpu().numpy()
+    ref = oracle.render(host, tab, -3.0, 8.0, (1, 1, 1), ocam(oracle, cs), W, H, 0.5, 0, 0.0)["rgba"]
+    assert np.abs(got - ref).max() <= TOL_EA
+    with pytest.raises(vr.VrError):
+        vol.vr_set_subcube((0, 0, 0), (71, 45, 52))
+    with pytest.raises(vr.VrError):
+        vol.vr_set_subcube((5, 0, 0), (4, 45, 52))
+    vol.close()
