@@ -297,8 +297,8 @@ __device__ __forceinline__ void classify_blend(const float4* __restrict__ tf, co
 }
 
 // ------------------------------------------------------------------------------------------------
-// a1 + a3 + a4/a5  the caster.  grid.x = sum over bricks of the 16x16-pixel tiles of their
-// rendering rectangles; block = 256 threads = 8 warps, each an 8x4-pixel patch.
+// a1 + a3 + a4/a5  the caster.  grid.x = sum over bricks of the CTA_W x CTA_H pixel tiles (16x8) of their
+// rendering rectangles; block = 128 threads = 4 warps, each an 8x4-pixel patch.
 // INSTR = 1 is the measuring build (samples evaluated, sector bitmap), never the product path.
 // ------------------------------------------------------------------------------------------------
 template <int MODE, int INSTR>
