@@ -148,6 +148,8 @@ def run_ours(args):
 
     w, views = workload_for(args)
     K, Wm = args.steps, args.warmup
+    if args.l2_fetch:
+        vr.vr_set_l2_fetch_granularity(args.l2_fetch)
     cube = w.cube("cuda")
     torch.cuda.synchronize()
     vol = vr.Volume(cube)
@@ -401,6 +403,8 @@ def main():
                     help="oracle legs render every n-th pixel in x and y (default 1 = the full frame for cpu_baseline, 4 for --impl reference)")
     ap.add_argument("--image", type=int, default=None, help="override the image size (W = H), e.g. 512 for Fig 12's comparison")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--l2-fetch", type=int, default=None, choices=[32, 64, 128],
+                    help="device-wide L2 fetch granularity hint in bytes (vr_set_l2_fetch_granularity); default: leave as is")
     ap.add_argument("--stage-times", action="store_true", help=argparse.SUPPRESS)
     ap.add_argument("--sweep", action="store_true", help="run BASELINE.json configs[4] (28 points) instead of the headline")
     args = ap.parse_args()

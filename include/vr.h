@@ -131,6 +131,20 @@ vr_status vr_plan_bricks(const int dims[3], const int bricks[3], const vr_camera
  *     Synchronises.  Either output may be NULL.                                                  */
 vr_status vr_measure(vr_volume* vol, const vr_camera* cam, int W, int H, float step_voxels, int mode,
                      float ert_alpha, long long* h_samples, long long* h_sectors);
+/* vr_measure_units: as vr_measure, with the distinct-unit count at three granularities: h_units[0] = 32-byte
+ *     sectors (= vr_measure's), h_units[1] = 64-byte sector pairs, h_units[2] = 128-byte lines that hold at least
+ *     one touched sector — the bytes a memory system fetching 64 or 128 bytes per miss has to move for the same
+ *     samples (decides between re-fetch and fetch granularity as the source of DRAM traffic
+ *     above the algorithmic bytes).  INVALID_ARG if h_units is NULL.                                            */
+vr_status vr_measure_units(vr_volume* vol, const vr_camera* cam, int W, int H, float step_voxels, int mode,
+                           float ert_alpha, long long* h_samples, long long h_units[3]);
+/* Device-wide hint for the number of bytes the L2 fetches from HBM per miss (cudaLimitMaxL2FetchGranularity):
+ *     32, 64 or 128.  The caster touches 32-byte sectors sparsely where rays are further apart than a voxel
+ *     (the step guarantees every voxel a ray intersects is sampled, not every voxel of the cube), so
+ *     the granularity decides how much untouched data rides along.  Affects the whole device (all volumes, all
+ *     other kernels of the process).  vr_get_... reads the current value.  INVALID_ARG for any other size.       */
+vr_status vr_set_l2_fetch_granularity(int bytes);
+vr_status vr_get_l2_fetch_granularity(int* h_bytes);
 /* Device time, in ms, of the cast kernel and of the composite kernel of the most recent vr_render /
  *     vr_render_to_host on this volume (CUDA events recorded on the volume's stream around each
  *     launch; composite is 0 when a single brick wrote the frame directly).  Waits for that frame. */

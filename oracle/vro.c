@@ -14,7 +14,10 @@
  *
  * Pins (tests/test_oracle_*.py, all -m "not gpu"): constant cube closed form, axis-aligned MIP
  * = max over an axis, axis-aligned EA = 1-D cumprod recurrence, continuous-limit integral of a
- * ramp, trilinear identities, brute force on tiny cubes, bricked = unbricked, symmetries.
+ * ramp, trilinear identities, brute force on tiny cubes, bricked = unbricked, symmetries; and, in
+ * tests/test_oracle_branches.py, the three branches a mutant once survived: the t_near >= 0 clamp (eye
+ * inside the box, box behind the eye), the d_a == 0 half-open containment rule (rays lying exactly on a
+ * face or brick plane) and the termination point (exact sample count of a terminated ray).
  * General oblique / perspective views of noisy cubes: PARITY UNPINNED beyond those invariants
  * (the oracle is the definition there) — stated in DESIGN.md as well.
  */
@@ -203,21 +206,15 @@ static int box_span(const double o[3], const double d[3], const double lo[3], co
     return *i_hi > *i_lo;
 }
 
+/* O9 for brick (bi,bj,bk) of the regular grid: its box, then box_span — the same code the renderer runs
+ * (route 1 below calls brick_box + box_span), so pins on this function pin the rendering path. */
 int vro_brick_span(const double o[3], const double d[3], const int dims[3], const int bricks[3],
                    int bi, int bj, int bk, double step, double t_near, double t_far,
                    double* t_in, long long* i_lo, long long* i_hi) {
     int idx[3] = {bi, bj, bk};
-    double lo[3], hi[3], t0, t1;
-    *t_in = 0.0; *i_lo = 0; *i_hi = 0;
+    double lo[3], hi[3];
     brick_box(dims, bricks, idx, lo, hi);
-    if (!vro_slab(o, d, lo, hi, &t0, &t1)) return 0;
-    if (t0 < t_near) t0 = t_near;
-    if (t1 > t_far) t1 = t_far;
-    if (!(t1 > t0)) return 0;
-    *t_in = t0;
-    *i_lo = lattice_index(t0, t_near, step);
-    *i_hi = lattice_index(t1, t_near, step);
-    return *i_hi > *i_lo;
+    return box_span(o, d, lo, hi, step, t_near, t_far, t_in, i_lo, i_hi);
 }
 
 /* ---------------------------------------------------------------- O5-O8 sample loop ------- */

@@ -48,6 +48,7 @@ struct FrameParams {
     float ert;                                // O7 threshold
     float x_zero_below;                       // table position below which alpha is exactly 0 (-1: nowhere)
     int ert_on;
+    int pf_every, pf_ahead;                   // L2 tile prefetch: every pf_every samples (power of two, 0 = off), pf_ahead samples ahead
 };
 
 struct BrickRec {
@@ -401,7 +402,34 @@ cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ 
         const unsigned slab_bytes = P.slab_stride * 4u;
         float vprev = sample_cached(vol_base, P.ty_stride, slab_bytes, nxm1, nym1, nzm1, q0x, q0y, q0z, K);
         bool done = false;
+#ifdef VR_EXP_L2PREFETCH
+        // EXPERIMENT (rejected, profiles/r02_experiments.md; build with VR_DEFINES=-DVR_EXP_L2PREFETCH, run with
+        // VR_PF=every,ahead): L2 tile prefetch.  Every pf_every samples the ray looks pf_ahead samples ahead and, when
+        // that point lies in an 8^3 tile it has not asked for yet, has the bulk-copy engine pull the whole 2 KB
+        // tile into the L2 (cp.async.bulk.prefetch.L2: one request per tile instead of one per 32-byte sector,
+        // and the row loads that follow find L2 latency instead of HBM latency).  Lanes of the warp that want the same
+        // tile are merged with match.any.  Purely a hint: no effect on any value.
+        unsigned pf_last = 0xffffffffu;
+        const unsigned pf_mask = (unsigned)P.pf_every - 1u;
+        const unsigned tiles_row = P.ty_stride >> 9, tiles_slab = P.slab_stride >> 9;
+#endif
         for (int j = 1; j < n; ++j) {
+#ifdef VR_EXP_L2PREFETCH
+            if (P.pf_every && ((unsigned)j & pf_mask) == 0u && j + P.pf_ahead < n) {
+                const float ja = (float)(j + P.pf_ahead);
+                const float ax = fminf(fmaxf(fmaf(ja, hx, q0x), 0.0f), nxm1), ay = fminf(fmaxf(fmaf(ja, hy, q0y), 0.0f), nym1),
+                            az = fminf(fmaxf(fmaf(ja, hz, q0z), 0.0f), nzm1);
+                const unsigned tid = ((unsigned)az >> 3) * tiles_slab + ((unsigned)ay >> 3) * tiles_row + ((unsigned)ax >> 3);
+                if (tid != pf_last) {
+                    pf_last = tid;
+                    const unsigned peers = __match_any_sync(__activemask(), tid);
+                    if ((peers & ((1u << (threadIdx.x & 31)) - 1u)) == 0u) {
+                        const unsigned long long a = vol_base + (unsigned long long)tid * (TILE_ELEMS * 4ull);
+                        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(a), "r"(TILE_ELEMS * 4) : "memory");
+                    }
+                }
+            }
+#endif
             const float jf = (float)j;
             const float v = sample_cached(vol_base, P.ty_stride, slab_bytes, nxm1, nym1, nzm1,
                                           fmaf(jf, hx, fmaf(jf, ex, q0x)), fmaf(jf, hy, fmaf(jf, ey, q0y)),
@@ -423,13 +451,23 @@ cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ 
     else img[pix] = M;
 }
 
-// number of set bits of the sector bitmap (measuring build only)
+// number of set bits of the sector bitmap (measuring build only): out[0] = distinct 32-byte sectors, out[1] = distinct
+// 64-byte units (sector pairs s, s^1) and out[2] = distinct 128-byte lines (sector quads) holding a touched sector —
+// what a memory system that fetches 64 or 128 bytes per miss would have to move for the same samples.
 __global__ void popcount_kernel(const unsigned* __restrict__ bitmap, size_t n_words, unsigned long long* out) {
-    unsigned long long c = 0;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_words; i += (size_t)gridDim.x * blockDim.x)
-        c += __popc(bitmap[i]);
-    for (int s = 16; s > 0; s >>= 1) c += __shfl_xor_sync(0xffffffffu, c, s);
-    if ((threadIdx.x & 31) == 0 && c) atomicAdd(out, c);
+    unsigned long long c32 = 0, c64 = 0, c128 = 0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_words; i += (size_t)gridDim.x * blockDim.x) {
+        const unsigned w = bitmap[i];
+        const unsigned p = (w | (w >> 1)) & 0x55555555u;          // bit 2k: pair k touched
+        const unsigned q = (p | (p >> 2)) & 0x11111111u;          // bit 4k: quad k touched
+        c32 += __popc(w); c64 += __popc(p); c128 += __popc(q);
+    }
+    for (int s = 16; s > 0; s >>= 1) {
+        c32 += __shfl_xor_sync(0xffffffffu, c32, s);
+        c64 += __shfl_xor_sync(0xffffffffu, c64, s);
+        c128 += __shfl_xor_sync(0xffffffffu, c128, s);
+    }
+    if ((threadIdx.x & 31) == 0 && c32) { atomicAdd(out, c32); atomicAdd(out + 1, c64); atomicAdd(out + 2, c128); }
 }
 
 // ------------------------------------------------------------------------------------------------

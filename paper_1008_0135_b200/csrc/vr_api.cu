@@ -5,6 +5,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -62,6 +63,7 @@ struct vr_volume {
     float* d_frame = nullptr;         // internal frame of vr_render_to_host
     size_t frame_floats = 0;
 
+    int pf_every = 0, pf_ahead = 0;   // L2 tile prefetch of the caster (0 = off); env VR_PF="every,ahead" overrides
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};   // cast begin/end, composite begin/end
     bool timed_cast = false, timed_comp = false;
 };
@@ -91,8 +93,8 @@ vr_status check_render_args(const vr_volume* vol, const vr_camera* cam, int W, i
 }
 
 // cropped = true: brick images are rect-sized and packed (vr_render); false: full W x H frames.
-void build_frame(const vr_volume* vol, const vr_camera* cam, int W, int H, float step, float ert, bool cropped,
-                 bool direct, Frame& f) {
+vr_status build_frame(const vr_volume* vol, const vr_camera* cam, int W, int H, float step, float ert, bool cropped,
+                      bool direct, Frame& f) {
     const vr::Basis bs = vr::make_basis(*cam);
     vr::FrameParams& P = f.P;
     for (int c = 0; c < 3; ++c) {
@@ -110,6 +112,7 @@ void build_frame(const vr_volume* vol, const vr_camera* cam, int W, int H, float
     P.inv_range = 1.0f / (vol->vmax - vol->vmin);
     P.ert_on = (ert > 0.0f && ert < 1.0f) ? 1 : 0;
     P.ert = ert;
+    P.pf_every = vol->pf_every; P.pf_ahead = vol->pf_ahead;
     {   // first table entry with alpha > 0 (the per-step correction keeps zeros zero)
         int j0 = 0;
         while (j0 < 256 && !(vol->tf_host[4 * j0 + 3] > 0.0f)) ++j0;
@@ -120,7 +123,7 @@ void build_frame(const vr_volume* vol, const vr_camera* cam, int W, int H, float
     vr::plan_bricks(vol->dims, vol->bricks, *cam, W, H, plan, f.order, vol->sub_lo, vol->sub_hi);
     const int B = (int)plan.size();
     f.recs.assign(B, vr::BrickRec());
-    int tiles = 0;
+    long long tiles = 0;                  // 64-bit: 512 full-frame rectangles at 32768^2 overflow an int
     size_t pool = 0;
     // CTAs are laid out brick by brick, front to back
     for (int k = 0; k < B; ++k) {
@@ -130,10 +133,10 @@ void build_frame(const vr_volume* vol, const vr_camera* cam, int W, int H, float
         vr::BrickRec& r = f.recs[b];
         for (int a = 0; a < 3; ++a) { r.lo[a] = bp.lo[a]; r.hi[a] = bp.hi[a]; }
         r.rx0 = bp.rx0; r.ry0 = bp.ry0; r.rw = bp.rw; r.rh = bp.rh;
-        r.tile0 = tiles;
+        r.tile0 = (int)std::min<long long>(tiles, 2147483647ll);
         r.tiles_x = (bp.rw + vr::CTA_W - 1) / vr::CTA_W;
         const int tiles_y = (bp.rh + vr::CTA_H - 1) / vr::CTA_H;
-        tiles += r.tiles_x * tiles_y;
+        tiles += (long long)r.tiles_x * tiles_y;
         if (cropped && !direct) {
             r.img_base = (long long)pool; r.img_stride = bp.rw; r.ox = bp.rx0; r.oy = bp.ry0;
             pool += (size_t)bp.rw * bp.rh;
@@ -142,8 +145,13 @@ void build_frame(const vr_volume* vol, const vr_camera* cam, int W, int H, float
         }
         r.pad = 0;
     }
-    f.total_tiles = tiles;
+    if (tiles > 2147483647ll)
+        return fail(VR_ERR_INVALID_ARG, "image x bricks too large: more than 2^31-1 pixel tiles in one frame");
+    if (pool > ((size_t)1 << 34))         // 16 Gi pixels of brick images = 256 GB of float4: cannot be meant
+        return fail(VR_ERR_INVALID_ARG, "image x bricks too large: brick images would exceed 2^34 pixels");
+    f.total_tiles = (int)tiles;
     f.pool_pixels = pool;
+    return VR_OK;
 }
 
 // The cast kernel looks its brick up by tile0 with a binary search over records in FRONT-TO-BACK order;
@@ -228,6 +236,12 @@ vr_status vr_create_volume(const int dims[3], const float* d_data, vr_volume** o
     vr_volume* v = new (std::nothrow) vr_volume();
     if (!v) return fail(VR_ERR_OOM, "vr_create_volume: host allocation failed");
     for (int a = 0; a < 3; ++a) { v->dims[a] = dims[a]; v->sub_hi[a] = dims[a]; }
+    if (const char* pf = std::getenv("VR_PF")) {           // tuning knob, see DESIGN.md "Kernels"
+        int ev_ = 0, ah = 0;
+        if (std::sscanf(pf, "%d,%d", &ev_, &ah) == 2 && ev_ >= 0 && ev_ <= 64 && (ev_ & (ev_ - 1)) == 0 && ah >= 0 && ah <= 256) {
+            v->pf_every = ev_; v->pf_ahead = ah;
+        }
+    }
     v->TX = (dims[0] + 1 + 7) / 8; v->TY = (dims[1] + 1 + 7) / 8; v->TZ = (dims[2] + 1 + 7) / 8;
     if ((double)v->TX * v->TY * vr::TILE_ELEMS >= 1073741824.0) {   // slab bytes and in-slab offsets stay 32-bit
         delete v;
@@ -236,7 +250,7 @@ vr_status vr_create_volume(const int dims[3], const float* d_data, vr_volume** o
     v->tiled_elems = (size_t)v->TX * v->TY * v->TZ * vr::TILE_ELEMS;
     cudaError_t e = cudaMalloc(&v->d_tiled, v->tiled_elems * sizeof(float));
     if (e == cudaSuccess) e = cudaMalloc(&v->d_range, 2 * vr::RANGE_SLOTS * sizeof(unsigned));
-    if (e == cudaSuccess) e = cudaMalloc(&v->d_tf_ea, 512 * sizeof(float4));
+    if (e == cudaSuccess) e = cudaMalloc(&v->d_tf_ea, 256 * sizeof(float4));
     if (e == cudaSuccess) e = cudaMalloc(&v->d_tf_raw, 256 * sizeof(float4));
     if (e == cudaSuccess) e = cudaMalloc(&v->d_bricks, VR_MAX_BRICKS * sizeof(vr::BrickRec));
     if (e == cudaSuccess) e = cudaMalloc(&v->d_order, VR_MAX_BRICKS * sizeof(int));
@@ -248,14 +262,16 @@ vr_status vr_create_volume(const int dims[3], const float* d_data, vr_volume** o
         dim3 grid((v->TX + 7) / 8, v->TY, v->TZ);
         std::vector<unsigned> init(2 * vr::RANGE_SLOTS);
         for (int k = 0; k < vr::RANGE_SLOTS; ++k) { init[2 * k] = 0xffffffffu; init[2 * k + 1] = 0u; }
-        cudaMemcpyAsync(v->d_range, init.data(), init.size() * sizeof(unsigned), cudaMemcpyHostToDevice, v->stream);
-        cudaEventRecord(e0, v->stream);
-        vr::relayout_kernel<<<grid, 256, 0, v->stream>>>(d_data, v->d_tiled, dims[0], dims[1], dims[2], v->TX, v->TY,
-                                                         v->d_range);
-        cudaEventRecord(e1, v->stream);
-        e = cudaGetLastError();
+        e = cudaMemcpyAsync(v->d_range, init.data(), init.size() * sizeof(unsigned), cudaMemcpyHostToDevice, v->stream);
+        if (e == cudaSuccess) e = cudaEventRecord(e0, v->stream);
+        if (e == cudaSuccess) {
+            vr::relayout_kernel<<<grid, 256, 0, v->stream>>>(d_data, v->d_tiled, dims[0], dims[1], dims[2], v->TX, v->TY,
+                                                             v->d_range);
+            e = cudaGetLastError();
+        }
+        if (e == cudaSuccess) e = cudaEventRecord(e1, v->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(v->stream);
-        if (e == cudaSuccess) cudaEventElapsedTime(&v->relayout_ms, e0, e1);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&v->relayout_ms, e0, e1);
         if (e == cudaSuccess) {
             std::vector<unsigned> slots(2 * vr::RANGE_SLOTS);
             e = cudaMemcpy(slots.data(), v->d_range, slots.size() * sizeof(unsigned), cudaMemcpyDeviceToHost);
@@ -348,22 +364,23 @@ vr_status vr_render(vr_volume* vol, const vr_camera* cam, int W, int H, float st
     const int B = vol->bricks[0] * vol->bricks[1] * vol->bricks[2];
     const bool direct = (B == 1 && mode == VR_MODE_EA);
     Frame f;
-    build_frame(vol, cam, W, H, step, ert, true, direct, f);
+    if ((s = build_frame(vol, cam, W, H, step, ert, true, direct, f)) != VR_OK) return s;
     if ((s = upload_plan(vol, f)) != VR_OK) return s;
     if (mode == VR_MODE_EA && (s = upload_tf_for_step(vol, (double)step)) != VR_OK) return s;
     vol->timed_cast = vol->timed_comp = false;
     if (!direct && (s = ensure_pool(vol, f.pool_pixels * (mode == VR_MODE_EA ? 4 : 1))) != VR_OK) return s;
-    cudaEventRecord(vol->ev[0], vol->stream);
+    VR_CUDA(cudaEventRecord(vol->ev[0], vol->stream), "record event");
     s = launch_cast<0>(vol, f, mode, direct ? d_out_rgba : vol->d_pool, nullptr, nullptr);
-    cudaEventRecord(vol->ev[1], vol->stream);
     if (s != VR_OK) return s;
+    VR_CUDA(cudaEventRecord(vol->ev[1], vol->stream), "record event");
     vol->timed_cast = true;
     if (direct) return VR_OK;
-    cudaEventRecord(vol->ev[2], vol->stream);
+    VR_CUDA(cudaEventRecord(vol->ev[2], vol->stream), "record event");
     s = launch_composite(vol, f, mode, vol->d_pool, W, H, d_out_rgba, d_out_scalar);
-    cudaEventRecord(vol->ev[3], vol->stream);
-    if (s == VR_OK) vol->timed_comp = true;
-    return s;
+    if (s != VR_OK) return s;
+    VR_CUDA(cudaEventRecord(vol->ev[3], vol->stream), "record event");
+    vol->timed_comp = true;
+    return VR_OK;
 }
 
 vr_status vr_get_stage_ms(vr_volume* vol, float* h_cast_ms, float* h_composite_ms) {
@@ -403,7 +420,7 @@ vr_status vr_render_bricks(vr_volume* vol, const vr_camera* cam, int W, int H, f
     if (s != VR_OK) return s;
     if (!d_brick_images) return fail(VR_ERR_INVALID_ARG, "vr_render_bricks: d_brick_images is NULL");
     Frame f;
-    build_frame(vol, cam, W, H, step, ert, false, false, f);
+    if ((s = build_frame(vol, cam, W, H, step, ert, false, false, f)) != VR_OK) return s;
     if ((s = upload_plan(vol, f)) != VR_OK) return s;
     if (mode == VR_MODE_EA && (s = upload_tf_for_step(vol, (double)step)) != VR_OK) return s;
     const size_t B = f.recs.size();
@@ -420,7 +437,7 @@ vr_status vr_composite(vr_volume* vol, const vr_camera* cam, int W, int H, int m
     if (s != VR_OK) return s;
     if (!d_brick_images || !d_out_rgba) return fail(VR_ERR_INVALID_ARG, "vr_composite: NULL image pointer");
     Frame f;
-    build_frame(vol, cam, W, H, 1.0f, 0.0f, false, false, f);
+    if ((s = build_frame(vol, cam, W, H, 1.0f, 0.0f, false, false, f)) != VR_OK) return s;
     // a stack of full frames may hold anything anywhere: composite every brick at every pixel
     for (auto& r : f.recs) { r.rx0 = 0; r.ry0 = 0; r.rw = W; r.rh = H; }
     if ((s = upload_plan(vol, f)) != VR_OK) return s;
@@ -448,12 +465,12 @@ vr_status vr_plan_bricks(const int dims[3], const int bricks[3], const vr_camera
     return VR_OK;
 }
 
-vr_status vr_measure(vr_volume* vol, const vr_camera* cam, int W, int H, float step, int mode, float ert,
-                     long long* h_samples, long long* h_sectors) {
+static vr_status measure_impl(vr_volume* vol, const vr_camera* cam, int W, int H, float step, int mode, float ert,
+                              long long* h_samples, long long h_units[3]) {
     vr_status s = check_render_args(vol, cam, W, H, step, mode);
     if (s != VR_OK) return s;
     Frame f;
-    build_frame(vol, cam, W, H, step, ert, true, false, f);
+    if ((s = build_frame(vol, cam, W, H, step, ert, true, false, f)) != VR_OK) return s;
     if ((s = upload_plan(vol, f)) != VR_OK) return s;
     if (mode == VR_MODE_EA && (s = upload_tf_for_step(vol, (double)step)) != VR_OK) return s;
     if ((s = ensure_pool(vol, f.pool_pixels * (mode == VR_MODE_EA ? 4 : 1))) != VR_OK) return s;
@@ -461,15 +478,17 @@ vr_status vr_measure(vr_volume* vol, const vr_camera* cam, int W, int H, float s
     unsigned* d_bitmap = nullptr;
     unsigned long long* d_cnt = nullptr;
     VR_CUDA(cudaMalloc(&d_bitmap, n_words * sizeof(unsigned)), "allocate sector bitmap");
-    cudaError_t e = cudaMalloc(&d_cnt, 2 * sizeof(unsigned long long));
+    cudaError_t e = cudaMalloc(&d_cnt, 4 * sizeof(unsigned long long));
     if (e != cudaSuccess) { cudaFree(d_bitmap); return cuda_fail(e, "allocate counters"); }
-    cudaMemsetAsync(d_bitmap, 0, n_words * sizeof(unsigned), vol->stream);
-    cudaMemsetAsync(d_cnt, 0, 2 * sizeof(unsigned long long), vol->stream);
-    s = launch_cast<1>(vol, f, mode, vol->d_pool, d_cnt, d_bitmap);
-    unsigned long long h[2] = {0, 0};
+    e = cudaMemsetAsync(d_bitmap, 0, n_words * sizeof(unsigned), vol->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(d_cnt, 0, 4 * sizeof(unsigned long long), vol->stream);
+    if (e != cudaSuccess) s = cuda_fail(e, "vr_measure: clear counters");
+    if (s == VR_OK) s = launch_cast<1>(vol, f, mode, vol->d_pool, d_cnt, d_bitmap);
+    unsigned long long h[4] = {0, 0, 0, 0};
     if (s == VR_OK) {
         vr::popcount_kernel<<<1184, 256, 0, vol->stream>>>(d_bitmap, n_words, d_cnt + 1);
-        e = cudaMemcpyAsync(h, d_cnt, sizeof(h), cudaMemcpyDeviceToHost, vol->stream);
+        e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaMemcpyAsync(h, d_cnt, sizeof(h), cudaMemcpyDeviceToHost, vol->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(vol->stream);
         if (e != cudaSuccess) s = cuda_fail(e, "vr_measure");
     }
@@ -477,7 +496,36 @@ vr_status vr_measure(vr_volume* vol, const vr_camera* cam, int W, int H, float s
     cudaFree(d_cnt);
     if (s != VR_OK) return s;
     if (h_samples) *h_samples = (long long)h[0];
-    if (h_sectors) *h_sectors = (long long)h[1];
+    if (h_units) for (int k = 0; k < 3; ++k) h_units[k] = (long long)h[1 + k];
+    return VR_OK;
+}
+
+vr_status vr_measure(vr_volume* vol, const vr_camera* cam, int W, int H, float step, int mode, float ert,
+                     long long* h_samples, long long* h_sectors) {
+    long long u[3] = {0, 0, 0};
+    vr_status s = measure_impl(vol, cam, W, H, step, mode, ert, h_samples, u);
+    if (s == VR_OK && h_sectors) *h_sectors = u[0];
+    return s;
+}
+
+vr_status vr_measure_units(vr_volume* vol, const vr_camera* cam, int W, int H, float step, int mode, float ert,
+                           long long* h_samples, long long h_units[3]) {
+    if (!h_units) return fail(VR_ERR_INVALID_ARG, "vr_measure_units: h_units is NULL");
+    return measure_impl(vol, cam, W, H, step, mode, ert, h_samples, h_units);
+}
+
+vr_status vr_set_l2_fetch_granularity(int bytes) {
+    if (bytes != 32 && bytes != 64 && bytes != 128)
+        return fail(VR_ERR_INVALID_ARG, "vr_set_l2_fetch_granularity: bytes must be 32, 64 or 128");
+    VR_CUDA(cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)bytes), "cudaDeviceSetLimit(L2 fetch granularity)");
+    return VR_OK;
+}
+
+vr_status vr_get_l2_fetch_granularity(int* h_bytes) {
+    if (!h_bytes) return fail(VR_ERR_INVALID_ARG, "vr_get_l2_fetch_granularity: NULL argument");
+    size_t v = 0;
+    VR_CUDA(cudaDeviceGetLimit(&v, cudaLimitMaxL2FetchGranularity), "cudaDeviceGetLimit(L2 fetch granularity)");
+    *h_bytes = (int)v;
     return VR_OK;
 }
 

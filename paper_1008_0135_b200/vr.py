@@ -19,7 +19,8 @@ VR_MAX_BRICKS = 512
 
 SYMBOLS = ["vr_create_volume", "vr_destroy_volume", "vr_set_stream", "vr_set_transfer_function",
            "vr_set_bricks", "vr_set_subcube", "vr_render", "vr_render_to_host", "vr_render_bricks", "vr_composite",
-           "vr_plan_bricks", "vr_measure", "vr_get_stage_ms", "vr_volume_info", "vr_volume_range", "vr_export_linear", "vr_last_error"]
+           "vr_plan_bricks", "vr_measure", "vr_measure_units", "vr_set_l2_fetch_granularity",
+           "vr_get_l2_fetch_granularity", "vr_get_stage_ms", "vr_volume_info", "vr_volume_range", "vr_export_linear", "vr_last_error"]
 
 
 class vr_camera(C.Structure):
@@ -60,6 +61,10 @@ def lib():
         L.vr_plan_bricks.argtypes = [ip, ip, cam, C.c_int, C.c_int, vp, ip]
         L.vr_measure.argtypes = [vp, cam, C.c_int, C.c_int, C.c_float, C.c_int, C.c_float,
                                  C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
+        L.vr_measure_units.argtypes = [vp, cam, C.c_int, C.c_int, C.c_float, C.c_int, C.c_float,
+                                       C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
+        L.vr_set_l2_fetch_granularity.argtypes = [C.c_int]
+        L.vr_get_l2_fetch_granularity.argtypes = [ip]
         L.vr_get_stage_ms.argtypes = [vp, fp, fp]
         L.vr_volume_info.argtypes = [vp, fp, C.POINTER(C.c_longlong)]
         L.vr_volume_range.argtypes = [vp, fp, fp]
@@ -80,6 +85,16 @@ def vr_last_error():
 def _check(status):
     if status != VR_OK:
         raise VrError(status, vr_last_error())
+
+
+def vr_set_l2_fetch_granularity(nbytes):
+    _check(lib().vr_set_l2_fetch_granularity(int(nbytes)))
+
+
+def vr_get_l2_fetch_granularity():
+    v = C.c_int(0)
+    _check(lib().vr_get_l2_fetch_granularity(C.byref(v)))
+    return v.value
 
 
 def make_camera(view, projection, fovy_deg=45.0, ortho_half_h=1.0):
@@ -205,6 +220,13 @@ class Volume:
         _check(lib().vr_measure(self._h, C.byref(cam), int(W), int(H), float(step), int(mode),
                                 float(ert_alpha), C.byref(s), C.byref(k)))
         return s.value, k.value
+
+    def vr_measure_units(self, cam, W, H, step, mode, ert_alpha=0.0):
+        """(samples evaluated, [distinct 32-byte sectors, 64-byte pairs, 128-byte lines] touched)."""
+        s, u = C.c_longlong(0), (C.c_longlong * 3)(0, 0, 0)
+        _check(lib().vr_measure_units(self._h, C.byref(cam), int(W), int(H), float(step), int(mode),
+                                      float(ert_alpha), C.byref(s), u))
+        return s.value, [int(u[0]), int(u[1]), int(u[2])]
 
     def vr_get_stage_ms(self):
         """(cast ms, composite ms) of the most recent vr_render; waits for it."""

@@ -49,8 +49,11 @@ def box_hits_by_faces(o, d, lo, hi, eps=1e-9):
     return min(ts), max(ts)
 
 
-def independent_pixel(cube, table, vmin, vmax, cs, W, H, step, mode, px, py):
-    """(rgba, scalar, n_samples) of one pixel, no bricks, no early termination."""
+def independent_pixel(cube, table, vmin, vmax, cs, W, H, step, mode, px, py, ert=0.0):
+    """(rgba, scalar, n_samples) of one pixel, no bricks.  ert in (0,1): the ray stops after the FIRST sample
+    whose accumulated opacity 1 - prod(1 - a) reaches ert (O7) and n_samples counts the samples up to and
+    including that one; n_samples is -1 when some partial opacity lies within 1e-9 of ert (the crossing sample
+    is then not decidable independently of the rounding order)."""
     nz, ny, nx = cube.shape
     o, d = pixel_ray_linalg(cs, W, H, px, py)
     hit = box_hits_by_faces(o, d, np.zeros(3), np.array([nx, ny, nz], dtype=np.float64))
@@ -78,7 +81,17 @@ def independent_pixel(cube, table, vmin, vmax, cs, W, H, step, mode, px, py):
         return rgba, M, len(ts)
     rgb = np.stack([np.interp(vals, xp, tab[:, c]) for c in range(3)], axis=1)
     a = np.interp(vals, xp, 1.0 - (1.0 - tab[:, 3]) ** step)
+    n_taken = len(ts)
+    if 0.0 < ert < 1.0:
+        A_run = 1.0 - np.cumprod(1.0 - a)
+        if np.any(np.abs(A_run - ert) < 1e-9):
+            n_taken = -1
+        else:
+            hit = np.nonzero(A_run >= ert)[0]
+            if hit.size:
+                n_taken = int(hit[0]) + 1
+                a, rgb = a[:n_taken], rgb[:n_taken]
     trans = np.concatenate([[1.0], np.cumprod(1.0 - a)[:-1]])
     C = (trans[:, None] * a[:, None] * rgb).sum(axis=0)
     A = 1.0 - np.prod(1.0 - a)
-    return np.array([C[0], C[1], C[2], A]), None, len(ts)
+    return np.array([C[0], C[1], C[2], A]), None, n_taken

@@ -24,7 +24,7 @@ def vr():
 def declared_symbols():
     text = open(os.path.join(ROOT, "include", "vr.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(vr_[a-z_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(vr_[a-z0-9_]+)\s*\(", text)))
 
 
 def test_header_symbols_exported(vr):
@@ -56,6 +56,9 @@ def test_null_and_range_checks_without_device(vr):
     assert L.vr_render(None, C.byref(cam), 8, 8, 1.0, 0, 0.0, None, None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_render_to_host(None, C.byref(cam), 8, 8, 1.0, 0, 0.0, None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_measure(None, C.byref(cam), 8, 8, 1.0, 0, 0.0, None, None) == vr.VR_ERR_INVALID_ARG
+    assert L.vr_measure_units(None, C.byref(cam), 8, 8, 1.0, 0, 0.0, None, None) == vr.VR_ERR_INVALID_ARG
+    assert L.vr_set_l2_fetch_granularity(48) == vr.VR_ERR_INVALID_ARG
+    assert L.vr_get_l2_fetch_granularity(None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_volume_info(None, None, None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_export_linear(None, None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_volume_range(None, None, None) == vr.VR_ERR_INVALID_ARG
