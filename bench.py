@@ -35,9 +35,12 @@ from paper_1008_0135_b200 import workloads as wl
 
 METRIC = "ms_per_frame_1024x1024"
 UNIT = "ms/frame"
-# Per-launch DRAM traffic of cast_kernel<EA> from the committed `ncu --set full` capture
-# (dram__bytes_read.sum + dram__bytes_write.sum, mean of the two r01d launches in profiles/r01cd_cast_full.md).
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 27.19e9
+# Per-launch DRAM traffic of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum of one
+# `ncu --set full` capture), keyed by the run it was captured on; any other run reports traffic = null.
+NCU_TRAFFIC = {
+    # (config, image, mode, bricks): (bytes per launch, profiles/ file the number comes from)
+    (3, 1024, 0, (2, 2, 2)): (27.19e9, "profiles/r01cd_cast_full.md (r01d, mean of launches az 10 / 20 deg)"),
+}
 
 
 def env_int(name, default):
@@ -123,6 +126,7 @@ def describe(w, views):
             "n_bricks": B, "image": f"{w.W}x{w.H}", "projection": "perspective45" if w.projection else "orthographic",
             "step_voxels": w.step, "mode": "EA" if w.mode == 0 else "MIP", "ert_alpha": w.ert_alpha,
             "views": f"{len(views)}-view orbit about y, el {w.el_deg} deg" if len(views) > 1 else f"az {w.az_deg} el {w.el_deg}",
+            "views_timed": None,
             "l2": "cube >> 126 MB L2: inputs larger than L2, no flush" if w.dims[0] * w.dims[1] * w.dims[2] * 4 > 4e8
                   else "cube fits L2; 512 MB scratch written between frames to flush it"}
 
@@ -188,9 +192,6 @@ def run_ours(args):
         ev[2 * k].record()
         vol.vr_render(cams[view_of(k)], w.W, w.H, w.step, w.mode, w.ert_alpha, out=out)
         ev[2 * k + 1].record()
-        if args.stage_times:                                      # waits for the frame: off by default
-            c, m = vol.vr_get_stage_ms()
-            cast_ms.append(c); comp_ms.append(m)
     barrier()
     t_wall1 = time.time()
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
@@ -267,10 +268,14 @@ def run_ours(args):
                   "gate": 5e-3 if w.ert_alpha > 0 else 1e-4}
         del host_cube
 
+    traffic, traffic_src = NCU_TRAFFIC.get((args.config, w.W if w.W == w.H else -1, w.mode, tuple(w.bricks)), (None, None))
+    cfg = describe(w, views)
+    cfg["views_timed"] = {"count": len(used_views), "azimuths_deg": [views[v] for v in used_views],
+                          "note": "view k of the timed region is azimuth views[k mod len(views)]; steps < len(views) time a prefix of the orbit"}
     line = {
         "metric": METRIC, "value": ms_per_frame, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
         "ms_per_step": total_ms / K, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32", "data": "synthetic", "config": describe(w, views),
+        "dtype": "f32", "data": "synthetic", "config": cfg,
         "frames_per_s_all_gpus": world * K / (total_ms * 1e-3),
         "ms_per_frame_min": min(per_frame), "ms_per_frame_max": max(per_frame),
         "ms_per_view": {str(int(views[view_of(k)])): round(per_frame[k], 3) for k in range(K)},
@@ -286,7 +291,7 @@ def run_ours(args):
         "gpu_launches": 2 * K if B > 1 or w.mode == 1 else K,
         "roofline": {"bound": "hbm", "kernel": "cast_kernel<EA>" if w.mode == 0 else "cast_kernel<MIP>",
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH, "peak_source": peak_src,
+                     "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": alg_bytes / K,
                      "cube_bytes": 4.0 * cube.numel(), "avg_launch_ms": cast_total_ms / K,
                      "definition": "32 B x distinct sectors of the tiled cube touched by the frame's samples "
@@ -334,9 +339,12 @@ def run_reference(args):
     ms = dt * 1e3 / K / frac
     sample = (f"each step: every {stride}th pixel in x and y of one orbit view ({px.size} rays), time scaled by "
               f"{1 / frac:g} to a full frame")
+    cfg = describe(w, views)
+    timed = sorted(set(k % len(views) for k in range(K)))
+    cfg["views_timed"] = {"count": len(timed), "azimuths_deg": [views[v] for v in timed]}
     line = {"impl": "reference", "metric": METRIC, "value": ms, "unit": UNIT, "n_gpus": args.gpus, "steps": K,
             "warmup": Wm, "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic", "config": describe(w, views),
+            "dtype": "f64", "data": "synthetic", "config": cfg,
             "cpu_baseline": {"value": ms, "unit": UNIT, "kind": "oracle", "cores": vro.max_threads(), "sample": sample,
                              "msamples_per_s": samples / dt / 1e6},
             "e2e": {"value": ms, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -360,6 +368,11 @@ def run_sweep(args):
     cam = vr.camera_from_spec(cs)
     peak, peak_src = measured_peak_gbs()
     reps = max(3, min(args.steps, 10))
+    host_cube, ocam = None, None
+    if not args.no_cpu_baseline:                                   # parity per point against the oracle (128x128-pixel lattice)
+        from oracle import vro
+        host_cube = cube.cpu().numpy()
+        ocam = vro.make_camera(cs.view, cs.projection, cs.fovy_deg, cs.ortho_half_h)
     for pt in wl.sweep_points():
         size, step, mode, bricks = pt["size"], pt["step"], pt["mode"], pt["bricks"]
         vol.vr_set_bricks(*bricks)
@@ -380,6 +393,15 @@ def run_sweep(args):
         best, med = ms[0], ms[len(ms) // 2]
         cast_med = sorted(cast)[len(cast) // 2]
         B = bricks[0] * bricks[1] * bricks[2]
+        parity = None
+        if host_cube is not None:
+            stride = size // 128
+            xs = np.arange(stride // 2, size, stride, dtype=np.int32)
+            yy, xx = np.meshgrid(xs, xs, indexing="ij")
+            px, py = xx.reshape(-1), yy.reshape(-1)
+            ref = vro.render_pixels(host_cube, w.table, w.vmin, w.vmax, bricks, ocam, size, size, step, mode, 0.0, 0, px, py)
+            got = out.cpu().numpy()[py, px]
+            parity = {"max_abs_err_vs_oracle": float(np.abs(got - ref["rgba"]).max()), "pixels": int(px.size), "gate": 1e-4}
         print(json.dumps({"sweep_point": {"mode": "MIP" if mode else "EA", "bricks": B, "step_voxels": step,
                                           "image": f"{size}x{size}"},
                           "ms_per_frame_best": best, "ms_per_frame_median": med, "cast_ms_median": cast_med,
@@ -387,7 +409,8 @@ def run_sweep(args):
                           "algorithmic_GB": 32e-9 * sectors, "bytes_per_sample": 32.0 * sectors / samples,
                           "hbm_GBps_algorithmic": 32e-9 * sectors / (cast_med * 1e-3),
                           "frac_of_peak": 32e-9 * sectors / (cast_med * 1e-3) / peak, "peak": peak,
-                          "side_of_ridge": "hbm" if 32.0 * sectors / samples > 14.0 else "alu/lsu"}), flush=True)
+                          "side_of_ridge": "hbm" if 32.0 * sectors / samples > 14.0 else "alu/lsu",
+                          "parity": parity}), flush=True)
         del out
     vol.close()
 
@@ -405,7 +428,6 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--l2-fetch", type=int, default=None, choices=[32, 64, 128],
                     help="device-wide L2 fetch granularity hint in bytes (vr_set_l2_fetch_granularity); default: leave as is")
-    ap.add_argument("--stage-times", action="store_true", help=argparse.SUPPRESS)
     ap.add_argument("--sweep", action="store_true", help="run BASELINE.json configs[4] (28 points) instead of the headline")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

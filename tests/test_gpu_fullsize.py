@@ -49,6 +49,13 @@ def gass(vr):
     vol.close()
 
 
+def report(tag, got, ref, gate):
+    """Print the measured per-channel margin (pytest -s / the captured log keeps it on record)."""
+    err = np.abs(np.asarray(got, dtype=np.float64) - ref).reshape(-1, ref.shape[-1] if ref.ndim > 1 else 1).max(axis=0)
+    print(f"[margin] {tag}: max abs err per channel {np.array2string(err, precision=3)} gate {gate:g} "
+          f"({err.max() / gate:.2f} of the gate)")
+
+
 def lattice(W, H, stride=8, offset=3):
     xs = np.arange(offset, W, stride, dtype=np.int32)
     ys = np.arange(offset, H, stride, dtype=np.int32)
@@ -71,6 +78,8 @@ def test_config3_full_size_sampled_pixels(vr, oracle, gass, az):
     got_off = vol.vr_render(cam, w.W, w.H, w.step, w.mode, 0.0).cpu().numpy()[py, px]
     got_on = vol.vr_render(cam, w.W, w.H, w.step, w.mode, w.ert_alpha).cpu().numpy()[py, px]
     assert ref_off[:, 3].max() > 0.5 and (ref_off[:, 3] > 0).mean() > 0.3       # a real picture
+    report(f"cfg3 az {az:g} ERT off", got_off, ref_off, 1e-4)
+    report(f"cfg3 az {az:g} ERT on vs oracle ERT on", got_on, ref_on, 5e-3)
     assert np.abs(got_off - ref_off).max() <= 1e-4, np.abs(got_off - ref_off).max(axis=0)
     assert np.abs(got_on - ref_off).max() <= 5e-3
     assert np.abs(got_on - ref_on).max() <= 5e-3
@@ -90,6 +99,7 @@ def test_config3_full_size_bricks_1_8_64_agree(vr, oracle, gass):
     for b in ((1, 1, 1), (2, 2, 2), (4, 4, 4)):
         vol.vr_set_bricks(*b)
         f = vol.vr_render(cam, w.W, w.H, w.step, w.mode, 0.0).cpu().numpy()
+        report(f"cfg3 az 40 bricks {b}", f[py, px], ref, 1e-4)
         assert np.abs(f[py, px] - ref).max() <= 1e-4, (b, np.abs(f[py, px] - ref).max(axis=0))
         frames.append(f)
     vol.vr_set_bricks(*w.bricks)
@@ -125,6 +135,48 @@ def test_full_size_ortho_sample_count_law(vr, gass):
     assert 0.5 * total_sectors < sectors <= total_sectors
 
 
+# ---- BASELINE.json configs[4]: the sweep's corners at full size (config 3's cube, ORTHO az 30 el 20, ERT off) ----
+@pytest.mark.parametrize("size,step,bricks", [(1024, 0.5, (2, 2, 2)), (1024, 0.25, (2, 2, 2)), (2048, 1.0, (2, 2, 2)),
+                                              (1024, 0.5, (4, 4, 4)), (512, 0.25, (1, 1, 1))])
+def test_config4_sweep_points_full_size(vr, oracle, gass, size, step, bricks):
+    """Step < 1 exercises what step 1 does not: the per-step opacity correction of the table (O6), the hi+lo
+    split of the fp32 step vector, several samples per voxel in the row cache (PAPER.md:185 sampling distance;
+    PAPER.md:207 output sizes).  16384-pixel lattice, gate 1e-4 per channel, margins printed."""
+    w, cube, host, vol = gass
+    cs = wl.orbit_camera(w.dims, 30.0, 20.0, wl.PROJ_ORTHO)
+    oc = oracle.make_camera(cs.view, cs.projection, cs.fovy_deg, cs.ortho_half_h)
+    px, py = lattice(size, size, stride=size // 128)
+    ref = oracle.render_pixels(host, w.table, w.vmin, w.vmax, bricks, oc, size, size, step, 0, 0.0, 0, px, py)["rgba"]
+    vol.vr_set_bricks(*bricks)
+    got = vol.vr_render(vr.camera_from_spec(cs), size, size, step, 0, 0.0).cpu().numpy()[py, px]
+    vol.vr_set_bricks(*w.bricks)
+    assert ref[:, 3].max() > 0.5
+    report(f"cfg4 EA {size}^2 step {step} bricks {bricks}", got, ref, 1e-4)
+    assert np.abs(got - ref).max() <= 1e-4, np.abs(got - ref).max(axis=0)
+
+
+def test_config4_mip_point_oblique_full_size(vr, oracle, gass):
+    """The sweep's MIP point (8 bricks, 1024^2, step 1) on the oblique az 30 / el 20 view: raw maxima within
+    1e-4 * max(1, |M|) of the oracle's, colours within 1e-4."""
+    import torch
+    w, cube, host, vol = gass
+    cs = wl.orbit_camera(w.dims, 30.0, 20.0, wl.PROJ_ORTHO)
+    oc = oracle.make_camera(cs.view, cs.projection, cs.fovy_deg, cs.ortho_half_h)
+    px, py = lattice(1024, 1024)
+    ref = oracle.render_pixels(host, w.table, w.vmin, w.vmax, w.bricks, oc, 1024, 1024, 1.0, 1, 0.0, 1, px, py)
+    sc = torch.empty((1024, 1024), dtype=torch.float32, device="cuda")
+    got = vol.vr_render(vr.camera_from_spec(cs), 1024, 1024, 1.0, 1, 0.0, out_scalar=sc).cpu().numpy()[py, px]
+    sc = sc.cpu().numpy()[py, px]
+    hit = np.isfinite(ref["scalar"])
+    assert hit.mean() > 0.3 and (np.isfinite(sc) == hit).all()
+    scale = np.maximum(1.0, np.abs(ref["scalar"][hit]))
+    rel = np.abs(sc[hit] - ref["scalar"][hit]) / scale
+    print(f"[margin] cfg4 MIP oblique: max |M - M_oracle| / max(1,|M|) = {rel.max():.3e} gate 1e-4; colours "
+          f"{np.abs(got - ref['rgba']).max():.3e}")
+    assert rel.max() <= 1e-4
+    assert np.abs(got - ref["rgba"]).max() <= 1e-4
+
+
 def test_config2_full_size_sampled_pixels(vr, oracle):
     """Config 2 (HIPASS-shaped 1721x1721x1024, 12.1 GB, orthographic, ERT off, piecewise table)."""
     import torch
@@ -143,4 +195,5 @@ def test_config2_full_size_sampled_pixels(vr, oracle):
     got = vol.vr_render(vr.camera_from_spec(cs), w.W, w.H, w.step, w.mode, 0.0).cpu().numpy()[py, px]
     vol.close()
     assert ref[:, 3].max() > 0.3
+    report("cfg2 full size", got, ref, 1e-4)
     assert np.abs(got - ref).max() <= 1e-4, np.abs(got - ref).max(axis=0)

@@ -114,7 +114,7 @@ def test_k_bricks_equal_unbricked(vr, oracle, bricks, proj):
     cube = wl.cube_blobs(dims, 11, "cuda", n_blobs=6, amp=6.0, sigma=5.0)
     cs = wl.orbit_camera(dims, 40.0, 25.0, proj)
     tab = wl.tf_ramp(0.15)
-    W, H = 150, 110                                       # not multiples of the 16x16 CTA tile
+    W, H = 150, 110                                       # not multiples of the 16x8-pixel CTA tile
     ref = oracle.render(cube.cpu().numpy(), tab, -3.0, 8.0, (1, 1, 1), ocam(oracle, cs), W, H, 0.5, 0, 0.0, route=0)["rgba"]
     got, _ = gpu_render(vr, cube, tab, -3.0, 8.0, bricks, cs, W, H, 0.5, 0, 0.0)
     assert np.abs(got - ref).max() <= TOL_EA, np.abs(got - ref).max(axis=(0, 1))
@@ -272,6 +272,79 @@ def test_measure_counts_every_sample_once(vr, oracle):
         assert samples == ref["samples"]
         total_sectors = -(-71 // 8) * -(-46 // 8) * -(-53 // 8) * 64
         assert 0 < sectors <= total_sectors
+
+
+def _footprint_units(oracle, dims, cs, W, H, step, eps):
+    """Distinct 32/64/128-byte units of the tiled cube (8^3 tiles, T_a = ceil((n_a+1)/8),
+    element index ((tz*TY + ty)*TX + tx)*512 + lz*64 + ly*8 + lx, sector = index >> 3) touched by the 2x2x2
+    footprints (i0, i0+1 per axis, i0 = floor(clamp(p - 1/2, 0, n-1))) of the ORACLE's sample positions
+    t_i = t_near + (i + 1/2) step, enumerated here in numpy.  Returns (must, may): `must` counts only footprints
+    whose floor is the same for any position error below eps voxels, `may` adds both candidates of the others —
+    the GPU computes positions in fp32 (error ~1e-5 voxel at these sizes), so its count lies in [must, may]."""
+    nx, ny, nz = dims
+    n_a = np.array([nx, ny, nz])
+    TX, TY = (nx + 8) // 8, (ny + 8) // 8
+    cam = oracle.make_camera(cs.view, cs.projection, cs.fovy_deg, cs.ortho_half_h)
+    must, may = [], []
+    for py in range(H):
+        for px in range(W):
+            o, d = oracle.ray(cam, W, H, px, py)
+            n, tn, tf = oracle.ray_extent(o, d, dims, step)
+            if n == 0:
+                continue
+            t = tn + (np.arange(n) + 0.5) * step
+            q = np.clip(o[None, :] + t[:, None] * d[None, :] - 0.5, 0.0, (n_a - 1)[None, :])
+            i0 = np.floor(q).astype(np.int64)
+            f = q - i0
+            lo_amb = (f < eps) & (i0 > 0)                       # could floor to i0 - 1
+            hi_amb = (f > 1.0 - eps) & (i0 < (n_a - 1)[None, :])  # could floor to i0 + 1
+            for shift, dest in ((0, must), (-1, None), (1, None)):
+                for corner in range(8):
+                    c = np.array([(corner >> a) & 1 for a in range(3)])
+                    v = i0 + c[None, :]
+                    if shift == 0:
+                        sel = np.ones(n, dtype=bool)
+                    else:
+                        amb = lo_amb if shift < 0 else hi_amb
+                        sel = amb.any(axis=1)
+                        if not sel.any():
+                            continue
+                        v = v + shift * amb
+                    x, y, z = v[sel, 0], v[sel, 1], v[sel, 2]
+                    idx = (((z >> 3) * TY + (y >> 3)) * TX + (x >> 3)) * 512 + (z & 7) * 64 + (y & 7) * 8 + (x & 7)
+                    (must if shift == 0 else may).append(idx >> 3)
+    must = np.unique(np.concatenate(must))
+    may = np.unique(np.concatenate([must] + may)) if may else must
+    def units(s):
+        return [np.unique(s >> k).size for k in (0, 1, 2)]
+    return units(must), units(may), must.size
+
+
+@pytest.mark.parametrize("proj,bricks,step,W,H", [(wl.PROJ_ORTHO, (1, 1, 1), 1.0, 40, 32), (wl.PROJ_PERSP, (2, 2, 2), 1.0, 36, 28),
+                                                  (wl.PROJ_ORTHO, (3, 1, 2), 0.5, 24, 20)])
+def test_measure_sector_count_equals_numpy_enumeration(vr, oracle, proj, bricks, step, W, H):
+    """The roofline numerator's instrument (vr_measure's sector bitmap, 32 B x distinct sectors) pinned against an
+    independent enumeration: numpy lists the footprints of the oracle's sample positions, maps them through the
+    documented tiled index and counts distinct 32-byte sectors, 64-byte pairs and 128-byte lines.  The images are
+    coarse (rays ~2-3 voxels apart) so that a good share of the sectors is NOT touched and a miscount shows."""
+    dims = (70, 45, 52)                                    # ragged: padding tiles on every axis
+    cube = wl.cube_blobs(dims, 11, "cuda", n_blobs=6, amp=6.0, sigma=5.0)
+    cs = wl.orbit_camera(dims, 40.0, 25.0, proj)
+    vol = vr.Volume(cube)
+    vol.vr_set_transfer_function(wl.tf_ramp(0.15), -3.0, 8.0)
+    vol.vr_set_bricks(*bricks)
+    samples, units = vol.vr_measure_units(vr.camera_from_spec(cs), W, H, step, 0, 0.0)
+    s2, sectors = vol.vr_measure(vr.camera_from_spec(cs), W, H, step, 0, 0.0)
+    s3, units_mip = vol.vr_measure_units(vr.camera_from_spec(cs), W, H, step, 1, 0.0)
+    vol.close()
+    must, may, _ = _footprint_units(oracle, dims, cs, W, H, step, eps=2e-4)
+    total = ((70 + 8) // 8) * ((45 + 8) // 8) * ((52 + 8) // 8) * 64
+    print(f"sectors gpu {units} numpy must {must} may {may} of {total}")
+    assert sectors == units[0] and s2 == samples == s3 and units_mip == units
+    assert must[0] < 0.9 * total                           # sparse enough to be a test
+    for k in range(3):
+        assert must[k] <= units[k] <= may[k], (k, must, units, may)
+        assert may[k] - must[k] <= max(2, 0.002 * must[k])  # the bracket is tight: equality up to a few ties
 
 
 def test_volume_range_equals_library_min_max(vr):
