@@ -86,6 +86,24 @@ vr_status vr_set_bricks(vr_volume* vol, int bx, int by, int bz);
  *     (S1).  NULL, NULL restores the whole cube.  INVALID_ARG unless 0 <= lo_a <= hi_a <= n_a.       */
 vr_status vr_set_subcube(vr_volume* vol, const int lo[3], const int hi[3]);
 
+/* NEXT-2  Empty-space skipping keyed to the transfer function ("keeping the size of these tasks
+ *     balanced"; PAPER.md:205 the work "varies based on the dataset characteristics"; PAPER.md:294 transfer functions
+ *     that suppress the noise).  The library keeps one bit per voxel cell (the unit cube between 8 neighbouring
+ *     voxel centres) saying whether a sample inside it can contribute under the current table: the bit is clear
+ *     when a corner is NaN (the sample is skipped, O5/A14) or when all 8 corners classify below the
+ *     table's first entry with alpha > 0 (the sample's alpha is exactly 0, O6/O7).  Emission-absorption rays pass
+ *     over such cells without reading the cube.  The frame is IDENTICAL to the one rendered without skipping —
+ *     only exactly-zero contributions are dropped — so this is a switch for measurements, not a quality setting.
+ *     The mask (1/32 of the cube) is rebuilt by one pass over the cube at the first emission-absorption render
+ *     after vr_set_transfer_function changed vmin, vmax or the length of the table's leading run of alpha = 0
+ *     (that render synchronises the stream); tables whose second entry already has alpha > 0, and MIP, do not
+ *     use it.  Default: enabled.
+ * vr_get_skip_info: builds the mask if it is due, then reports whether skipping is active for the current table,
+ *     the build time of the mask in ms, its size in bytes and the fraction of cells whose bit is set.            */
+vr_status vr_set_empty_space_skipping(vr_volume* vol, int enabled);
+vr_status vr_get_skip_info(vr_volume* vol, int* h_active, float* h_build_ms, long long* h_mask_bytes,
+                           double* h_occupied_fraction);
+
 /* a1-a7  One frame: per-brick ray casting inside each brick's rendering rectangle
  *     (PAPER.md:150), then depth-ordered composition into d_out_rgba.
  *     step_voxels: sampling distance along the ray in voxels, > 0.
@@ -126,18 +144,21 @@ vr_status vr_plan_bricks(const int dims[3], const int bricks[3], const vr_camera
 
 /* Measurement aids (not on the product path):
  * vr_measure: renders the frame with the instrumented build of the caster and returns, in HOST
- *     counters, the samples actually evaluated and the number of distinct 32-byte sectors of the
- *     tiled cube that the samples' 2x2x2 footprints touched (algorithmic HBM bytes = 32 * that).
+ *     counters, the lattice samples visited (every sample of O4 up to early termination: the oracle's
+ *     count) and the number of distinct 32-byte sectors of the tiled cube that the evaluated samples'
+ *     2x2x2 footprints touched (algorithmic HBM bytes of the cube = 32 * that).
  *     Synchronises.  Either output may be NULL.                                                  */
 vr_status vr_measure(vr_volume* vol, const vr_camera* cam, int W, int H, float step_voxels, int mode,
                      float ert_alpha, long long* h_samples, long long* h_sectors);
-/* vr_measure_units: as vr_measure, with the distinct-unit count at three granularities: h_units[0] = 32-byte
- *     sectors (= vr_measure's), h_units[1] = 64-byte sector pairs, h_units[2] = 128-byte lines that hold at least
- *     one touched sector — the bytes a memory system fetching 64 or 128 bytes per miss has to move for the same
- *     samples (decides between re-fetch and fetch granularity as the source of DRAM traffic
- *     above the algorithmic bytes).  INVALID_ARG if h_units is NULL.                                            */
+/* vr_measure_units: the full set of counters of the instrumented caster (which takes the same skip and termination
+ *     decisions as the product caster).  h_samples[0] = lattice samples visited (= vr_measure's, the oracle's
+ *     count), h_samples[1] = samples evaluated (visited minus those empty-space skipping passed over).
+ *     h_units[0..2] = distinct 32-byte sectors (= vr_measure's), 64-byte sector pairs and 128-byte lines of the
+ *     tiled cube that the EVALUATED samples' footprints touched — what a memory system fetching 32, 64 or 128
+ *     bytes per miss has to move; h_units[3] = distinct 32-byte sectors of the occupancy mask that were read.
+ *     Either array may be NULL.                                                                                 */
 vr_status vr_measure_units(vr_volume* vol, const vr_camera* cam, int W, int H, float step_voxels, int mode,
-                           float ert_alpha, long long* h_samples, long long h_units[3]);
+                           float ert_alpha, long long h_samples[2], long long h_units[4]);
 /* Device-wide hint for the number of bytes the L2 fetches from HBM per miss (cudaLimitMaxL2FetchGranularity):
  *     32, 64 or 128.  The caster touches 32-byte sectors sparsely where rays are further apart than a voxel
  *     (the step guarantees every voxel a ray intersects is sampled, not every voxel of the cube), so

@@ -48,7 +48,8 @@ struct FrameParams {
     float ert;                                // O7 threshold
     float x_zero_below;                       // table position below which alpha is exactly 0 (-1: nowhere)
     int ert_on;
-    int pf_every, pf_ahead;                   // L2 tile prefetch: every pf_every samples (power of two, 0 = off), pf_ahead samples ahead
+    int seg_len, seg_span;                    // samples per anchored segment; ceil(seg_len*step)+1 (sampler.cuh)
+    int nbx, nby;                             // occupancy-mask words (4^3 cells) per row / per column
 };
 
 struct BrickRec {
@@ -61,11 +62,14 @@ struct BrickRec {
 };
 
 // ------------------------------------------------------------------------------------------------
-// a0  re-layout.  One CTA moves an 8(z) x 8(y) x 64(x) block: coalesced row reads -> shared memory
-// -> 8 whole tiles written as one contiguous 16 KB run of float4 stores.  Source indices are
-// clamped, so the padding voxels replicate the cube's faces (this makes
-// x+1 / y+1 / z+1 of any in-range voxel addressable without a bounds test, with the same result as
-// the clamp of O5 because the weight of the replicated voxel is then exactly zero).
+// a0  re-layout.  The tiled copy holds the cube in PADDED coordinates u = voxel index + 1: one replicated layer
+// below index 0 and at least one above index n-1 on every axis (T_a = ceil((n_a + 2)/8) tiles).  Trilinear
+// interpolation between an edge voxel and its replica returns the edge value exactly (fma(f, v-v, v) = v), which is
+// O5's clamp-to-edge without a clamp, a floor of a negative number or a bounds test in the sample loop: a sample
+// at q = p - 1/2 in [-1/2, n - 1/2] reads padded cells floor(q + 1) in [0, n] and floor(q + 1) + 1 in [1, n + 1].
+// (An infinite voxel on a face would give inf - inf = NaN where the clamp gives inf; survey cubes blank with NaN.)
+// One CTA moves an 8(z) x 8(y) x 64(x) block: coalesced row reads -> shared memory -> 8 whole tiles written as
+// one contiguous 16 KB run of float4 stores.
 // ------------------------------------------------------------------------------------------------
 constexpr int RANGE_SLOTS = 256;
 // order-preserving map float -> unsigned (so atomicMin/atomicMax on the key order the floats)
@@ -93,13 +97,13 @@ relayout_kernel(const float* __restrict__ src, float* __restrict__ dst, int nx, 
     const int tx0 = blockIdx.x * 8, ty = blockIdx.y, tz = blockIdx.z;
     const int t = threadIdx.x;
     const int xo = t & 63;
-    const int xs = min(tx0 * 8 + xo, nx - 1);
+    const int xs = min(max(tx0 * 8 + xo - 1, 0), nx - 1);      // padded -> voxel, replicated at both ends
     float vmin = INFINITY, vmax = -INFINITY;
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
         const int row = (t >> 6) + 4 * k;
-        const int z = min(tz * 8 + (row >> 3), nz - 1);
-        const int y = min(ty * 8 + (row & 7), ny - 1);
+        const int z = min(max(tz * 8 + (row >> 3) - 1, 0), nz - 1);
+        const int y = min(max(ty * 8 + (row & 7) - 1, 0), ny - 1);
         const float val = __ldcs(src + ((size_t)z * ny + y) * nx + xs);
         sm[row][xo] = val;
         vmin = fminf(vmin, val);      // fminf/fmaxf ignore NaN (blanked voxels)
@@ -140,7 +144,7 @@ relayout_kernel(const float* __restrict__ src, float* __restrict__ dst, int nx, 
     }
 }
 
-// element offset of voxel (x,y,z) in the tiled copy
+// element offset of PADDED position (x,y,z) = voxel index + 1 in the tiled copy
 __device__ __forceinline__ size_t tiled_index(int x, int y, int z, unsigned ty_stride, unsigned slab_stride) {
     return (size_t)(z >> 3) * slab_stride + (size_t)(y >> 3) * ty_stride + (size_t)(x >> 3) * TILE_ELEMS +
            (size_t)(((z & 7) << 6) | ((y & 7) << 3) | (x & 7));
@@ -154,7 +158,7 @@ __global__ void export_linear_kernel(const float* __restrict__ tiled, float* __r
         const int x = (int)(i % nx);
         const size_t r = i / nx;
         const int y = (int)(r % ny), z = (int)(r / ny);
-        dst[i] = tiled[tiled_index(x, y, z, ty_stride, slab_stride)];
+        dst[i] = tiled[tiled_index(x + 1, y + 1, z + 1, ty_stride, slab_stride)];
     }
 }
 
@@ -214,28 +218,19 @@ __device__ __forceinline__ long long lattice_index(double t, double t_near, doub
 }
 
 // ------------------------------------------------------------------------------------------------
-// O5  trilinear sample of the tiled cube at (qx,qy,qz) = position - 1/2, fp32.
+// O5  plain 8-corner trilinear sample of one cell (measuring build only: marks the 32-byte sectors it reads).
 // ------------------------------------------------------------------------------------------------
-struct Footprint {           // the 8 voxels of one sample and its fractional weights
+struct Footprint {           // the 8 voxels of one sample
     float v[8];
-    float fx, fy, fz;
 };
 
-template <int INSTR>
-__device__ __forceinline__ void fetch(const float* __restrict__ vol, const FrameParams& P, float nxm1, float nym1,
-                                      float nzm1, float qx, float qy, float qz, Footprint& F,
-                                      unsigned* __restrict__ bitmap) {
-    qx = fminf(fmaxf(qx, 0.0f), nxm1);
-    qy = fminf(fmaxf(qy, 0.0f), nym1);
-    qz = fminf(fmaxf(qz, 0.0f), nzm1);
-    // floor of a non-negative float < 2^22 without F2I/I2F: add 2^23 rounding down, the integer is
-    // then the low mantissa bits and (r - 2^23) is that integer as a float, exactly.
-    const float rx = __fadd_rd(qx, 8388608.0f), ry = __fadd_rd(qy, 8388608.0f), rz = __fadd_rd(qz, 8388608.0f);
-    const unsigned ix = __float_as_uint(rx) & 0x7fffffu, iy = __float_as_uint(ry) & 0x7fffffu,
-                   iz = __float_as_uint(rz) & 0x7fffffu;
-    F.fx = qx - (rx - 8388608.0f);
-    F.fy = qy - (ry - 8388608.0f);
-    F.fz = qz - (rz - 8388608.0f);
+}  // namespace vr
+#include "sampler.cuh"
+namespace vr {
+
+__device__ __forceinline__ void fetch_marked(const float* __restrict__ vol, const FrameParams& P, const Cell& c,
+                                             Footprint& F, unsigned* __restrict__ bitmap) {
+    const unsigned ix = c.ix, iy = c.iy, iz = c.iz;
     // separable tiled offsets; +1 neighbours always exist (padding), see relayout_kernel
     const unsigned ix1 = ix + 1, iy1 = iy + 1, iz1 = iz + 1;
     const unsigned ex0 = (ix >> 3) * TILE_ELEMS + (ix & 7), ex1 = (ix1 >> 3) * TILE_ELEMS + (ix1 & 7);
@@ -247,32 +242,27 @@ __device__ __forceinline__ void fetch(const float* __restrict__ vol, const Frame
     F.v[2] = __ldg(pz0 + e01); F.v[3] = __ldg(pz0 + e11);
     F.v[4] = __ldg(pz1 + e00); F.v[5] = __ldg(pz1 + e10);
     F.v[6] = __ldg(pz1 + e01); F.v[7] = __ldg(pz1 + e11);
-    if (INSTR) {   // mark the 32-byte sectors (8 consecutive floats) of the footprint
-        const size_t b0 = (size_t)(pz0 - vol), b1 = (size_t)(pz1 - vol);
-        const size_t s[8] = {(b0 + e00) >> 3, (b0 + e10) >> 3, (b0 + e01) >> 3, (b0 + e11) >> 3,
-                             (b1 + e00) >> 3, (b1 + e10) >> 3, (b1 + e01) >> 3, (b1 + e11) >> 3};
+    // mark the 32-byte sectors (8 consecutive floats) of the footprint
+    const size_t b0 = (size_t)(pz0 - vol), b1 = (size_t)(pz1 - vol);
+    const size_t s[8] = {(b0 + e00) >> 3, (b0 + e10) >> 3, (b0 + e01) >> 3, (b0 + e11) >> 3,
+                         (b1 + e00) >> 3, (b1 + e10) >> 3, (b1 + e01) >> 3, (b1 + e11) >> 3};
 #pragma unroll
-        for (int k = 0; k < 8; ++k) {
-            const unsigned bit = 1u << (unsigned)(s[k] & 31);
-            unsigned* w = bitmap + (s[k] >> 5);
-            if (!(*(volatile unsigned*)w & bit)) atomicOr(w, bit);
-        }
+    for (int k = 0; k < 8; ++k) {
+        const unsigned bit = 1u << (unsigned)(s[k] & 31);
+        unsigned* w = bitmap + (s[k] >> 5);
+        if (!(*(volatile unsigned*)w & bit)) atomicOr(w, bit);
     }
 }
 
-__device__ __forceinline__ float trilerp(const Footprint& F) {
-    const float c00 = fmaf(F.fx, F.v[1] - F.v[0], F.v[0]);
-    const float c10 = fmaf(F.fx, F.v[3] - F.v[2], F.v[2]);
-    const float c01 = fmaf(F.fx, F.v[5] - F.v[4], F.v[4]);
-    const float c11 = fmaf(F.fx, F.v[7] - F.v[6], F.v[6]);
-    const float c0 = fmaf(F.fy, c10 - c00, c00);
-    const float c1 = fmaf(F.fy, c11 - c01, c01);
-    return fmaf(F.fz, c1 - c0, c0);
+__device__ __forceinline__ float trilerp(const Footprint& F, const Cell& c) {
+    const float c00 = fmaf(c.fx, F.v[1] - F.v[0], F.v[0]);
+    const float c10 = fmaf(c.fx, F.v[3] - F.v[2], F.v[2]);
+    const float c01 = fmaf(c.fx, F.v[5] - F.v[4], F.v[4]);
+    const float c11 = fmaf(c.fx, F.v[7] - F.v[6], F.v[6]);
+    const float c0 = fmaf(c.fy, c10 - c00, c00);
+    const float c1 = fmaf(c.fy, c11 - c01, c01);
+    return fmaf(c.fz, c1 - c0, c0);
 }
-
-}  // namespace vr
-#include "sampler.cuh"
-namespace vr {
 
 // O6 + O7: classify through the shared-memory table (256 float4 entries) and blend.
 // Transparent-sample skip: x_zero_below = (index of the first table entry with alpha > 0) - 1.  For x below it both
@@ -298,16 +288,80 @@ __device__ __forceinline__ void classify_blend(const float4* __restrict__ tf, co
 }
 
 // ------------------------------------------------------------------------------------------------
+// NEXT-2  occupancy mask for empty-space skipping (PAPER.md:144 balanced work, PAPER.md:205 finding 2: the work
+// depends on the data, PAPER.md:294 noise-suppressing transfer functions).  One bit per PADDED cell (i,j,k), i in
+// [0, n_x] etc. = the unit cube between padded voxels i..i+1, j..j+1, k..k+1 in which O5 interpolates (cell 0 and
+// cell n_a are the half-voxel rims where the replicated layer stands in for the clamp).  The bit is CLEAR when
+// every sample in the cell contributes exactly nothing under the current table:
+//   * a corner is NaN  -> the blend is NaN -> the sample is skipped (O5/A14), or
+//   * all 8 corners classify more than MASK_MARGIN table entries below the first entry with alpha > 0: the
+//     blend is a convex combination of the corners (up to a few ulp), so its table position x is below
+//     x_zero_below and both entries the lookup blends have alpha = 0 (O6) -> C and A unchanged (O7).
+// A clear bit therefore never changes a pixel: the oracle needs no rule for it, and parity gates stay as they are.
+// Layout: 64-bit words of 4x4x4 cells, word ((bz*NBY + by)*NBX + bx), bit (lz*4 + ly)*4 + lx.
+// One CTA = 32 x 8 x 8 cells (8 x 2 x 2 words): the 33 x 9 x 9 corner classes go through shared memory.
+// ------------------------------------------------------------------------------------------------
+constexpr float MASK_MARGIN = 0.01f;       // in table entries (x units): far above fp32 rounding of the blend
+
+__global__ void __launch_bounds__(256)
+build_mask_kernel(const float* __restrict__ vol, unsigned ty_stride, unsigned slab_stride, int nx, int ny, int nz,
+                  float vmin, float inv_range, float x_zero_below, unsigned long long* __restrict__ mask, int NBX,
+                  int NBY, unsigned long long* __restrict__ n_occupied) {
+    __shared__ unsigned char cls[9][9][36];    // 1 = may be visible, 2 = NaN
+    __shared__ unsigned words[2][2][8][2];     // [wz][wy][wx][half]
+    const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 8, z0 = blockIdx.z * 8;
+    const int t = threadIdx.x;
+    if (t < 64) (&words[0][0][0][0])[t] = 0u;
+    for (int i = t; i < 9 * 9 * 33; i += 256) {
+        const int lx = i % 33, r = i / 33, ly = r % 9, lz = r / 9;
+        const int x = min(x0 + lx, nx + 1), y = min(y0 + ly, ny + 1), z = min(z0 + lz, nz + 1);   // padded coordinates
+        const float v = __ldg(vol + tiled_index(x, y, z, ty_stride, slab_stride));
+        const float xt = __saturatef((v - vmin) * inv_range) * 255.0f;
+        cls[lz][ly][lx] = (v != v) ? 2 : (xt < x_zero_below - MASK_MARGIN ? 0 : 1);
+    }
+    __syncthreads();
+    const int lz = t >> 5, ly = (t >> 2) & 7, lxq = (t & 3) * 8;
+    unsigned bits = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const int lx = lxq + k;
+        const unsigned o = cls[lz][ly][lx] | cls[lz][ly][lx + 1] | cls[lz][ly + 1][lx] | cls[lz][ly + 1][lx + 1] |
+                           cls[lz + 1][ly][lx] | cls[lz + 1][ly][lx + 1] | cls[lz + 1][ly + 1][lx] | cls[lz + 1][ly + 1][lx + 1];
+        const bool in = (x0 + lx <= nx) && (y0 + ly <= ny) && (z0 + lz <= nz);      // n_a + 1 cells per axis
+        if (in && (o & 1u) && !(o & 2u)) bits |= 1u << k;
+    }
+    // bits 0..3 -> word wx = 2*(t&3), bits 4..7 -> word wx + 1; bit position in the word: (lz&3)*16 + (ly&3)*4 + lx&3
+    const int wz = lz >> 2, wy = ly >> 2, pos = ((lz & 3) << 4) | ((ly & 3) << 2);
+    const unsigned lo4 = bits & 15u, hi4 = bits >> 4;
+    if (lo4) atomicOr(&words[wz][wy][2 * (t & 3)][pos >> 5], lo4 << (pos & 31));
+    if (hi4) atomicOr(&words[wz][wy][2 * (t & 3) + 1][pos >> 5], hi4 << (pos & 31));
+    __syncthreads();
+    if (t < 32) {
+        const int wx = t & 7, wyy = (t >> 3) & 1, wzz = t >> 4;
+        const int bx = blockIdx.x * 8 + wx, by = blockIdx.y * 2 + wyy, bz = blockIdx.z * 2 + wzz;
+        const unsigned long long w = (unsigned long long)words[wzz][wyy][wx][0] | ((unsigned long long)words[wzz][wyy][wx][1] << 32);
+        const bool in = bx < NBX && by < NBY && bz * 4 <= nz;
+        if (in) mask[((size_t)bz * NBY + by) * NBX + bx] = w;
+        unsigned long long cnt = in ? (unsigned long long)__popcll(w) : 0ull;
+        for (int sft = 16; sft > 0; sft >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, sft);
+        if (t == 0 && cnt) atomicAdd(n_occupied, cnt);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // a1 + a3 + a4/a5  the caster.  grid.x = sum over bricks of the CTA_W x CTA_H pixel tiles (16x8) of their
 // rendering rectangles; block = 128 threads = 4 warps, each an 8x4-pixel patch.
-// INSTR = 1 is the measuring build (samples evaluated, sector bitmap), never the product path.
+// SKIP = 1 consults the occupancy mask (EA only).  INSTR = 1 is the measuring build (samples, sector bitmaps),
+// never the product path; it walks the same cells and takes the same skip and termination decisions.
+// counters (INSTR): [0] lattice samples visited (the oracle's count), [1] samples evaluated (not skipped).
 // ------------------------------------------------------------------------------------------------
-template <int MODE, int INSTR>
+template <int MODE, int INSTR, int SKIP>
 __global__ void __launch_bounds__(CTA_THREADS, VR_CAST_MINBLOCKS)
 cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ bricks, int n_bricks,
-            const float* __restrict__ vol, const float4* __restrict__ tf_global, float* __restrict__ img,
-            unsigned long long* __restrict__ counters, unsigned* __restrict__ bitmap) {
-        __shared__ __align__(16) float4 tf[MODE == MODE_EA ? 256 : 1];   // 4 KB: keeps the L1 share of the SM large
+            const float* __restrict__ vol, const float4* __restrict__ tf_global, const unsigned long long* __restrict__ mask,
+            float* __restrict__ img, unsigned long long* __restrict__ counters, unsigned* __restrict__ bitmap,
+            unsigned* __restrict__ mask_bitmap) {
+    __shared__ __align__(16) float4 tf[MODE == MODE_EA ? 256 : 1];   // 4 KB: keeps the L1 share of the SM large
     __shared__ int s_brick;
     if (MODE == MODE_EA) {
         for (int i = threadIdx.x; i < 256; i += CTA_THREADS) tf[i] = tf_global[i];
@@ -366,83 +420,101 @@ cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ 
         else img[pix] = -INFINITY;
         return;
     }
-    // anchor the brick's first sample in double, then march in fp32: q_j = q0 + j*ds  (q = position - 1/2)
-    const double ta = t_near + ((double)i_lo + 0.5) * P.step;
-    const float q0x = (float)(o[0] + ta * d[0] - 0.5), q0y = (float)(o[1] + ta * d[1] - 0.5),
-                q0z = (float)(o[2] + ta * d[2] - 0.5);
-    const double dsx = P.step * d[0], dsy = P.step * d[1], dsz = P.step * d[2];
-    const float hx = (float)dsx, hy = (float)dsy, hz = (float)dsz;                 // step vector, high part
-    const float ex = (float)(dsx - (double)hx), ey = (float)(dsy - (double)hy), ez = (float)(dsz - (double)hz);
-    const float nxm1 = (float)(P.nx - 1), nym1 = (float)(P.ny - 1), nzm1 = (float)(P.nz - 1);
+    // The march: segments of P.seg_len (<= 64) samples, each anchored in double (sampler.cuh); inside a segment
+    // u_rel(j') = rel + j' h in fp32.  With empty-space skipping a segment is walked twice: an occupancy pass
+    // that only locates each sample's cell and collects one bit per sample from the mask, then the sampling pass
+    // over the set bits — lanes of a warp then work on different samples of the SAME segment, which compacts the
+    // occupied samples of 32 rays into full warp instructions without letting the rays drift apart.
+    const float h[3] = {(float)(P.step * d[0]), (float)(P.step * d[1]), (float)(P.step * d[2])};
+    const unsigned nbx = (unsigned)P.nbx, nbxy = (unsigned)P.nbx * (unsigned)P.nby;
 
     float Cr = 0.f, Cg = 0.f, Cb = 0.f, A = 0.f, M = -INFINITY;
-    unsigned long long count = 0;
+    MaskCursor mc;
+    mc.lo = mc.hi = 0u; mc.tag = 0xffffffffu;
     if (INSTR) {
-        for (int j = 0; j < n; ++j) {
-            const float jf = (float)j;
-            Footprint F;
-            fetch<1>(vol, P, nxm1, nym1, nzm1, fmaf(jf, hx, fmaf(jf, ex, q0x)), fmaf(jf, hy, fmaf(jf, ey, q0y)),
-                     fmaf(jf, hz, fmaf(jf, ez, q0z)), F, bitmap);
-            const float v = trilerp(F);
-            ++count;
-            if (MODE == MODE_EA) {
-                classify_blend(tf, P, v, Cr, Cg, Cb, A);
-                if (P.ert_on && A >= P.ert) break;
-            } else {
-                M = fmaxf(M, v);
+        unsigned long long visited = 0, evaluated = 0;
+        bool done = false;
+        for (int js = 0; js < n && !done; js += P.seg_len) {
+            Anchor An;
+            set_anchor(o, d, t_near, P.step, i_lo + js, h, P.seg_span, An);
+            const int je = min(n - js, P.seg_len);
+            for (int jl = 0; jl < je; ++jl) {
+                Cell c;
+                locate(An, jl, h, c);
+                ++visited;
+                if (SKIP) {
+                    const unsigned tag = (c.iz >> 2) * nbxy + (c.iy >> 2) * nbx + (c.ix >> 2);
+                    if (mask_bitmap) {             // 32-byte sectors of the mask = 4 words
+                        const unsigned sct = tag >> 2, bit = 1u << (sct & 31);
+                        if (!(*(volatile unsigned*)(mask_bitmap + (sct >> 5)) & bit)) atomicOr(mask_bitmap + (sct >> 5), bit);
+                    }
+                    if (!cell_occupied(mask, nbx, nbxy, c.ix, c.iy, c.iz, mc)) continue;
+                }
+                Footprint F;
+                fetch_marked(vol, P, c, F, bitmap);
+                const float v = trilerp(F, c);
+                ++evaluated;
+                if (MODE == MODE_EA) {
+                    classify_blend(tf, P, v, Cr, Cg, Cb, A);
+                    if (P.ert_on && A >= P.ert) { done = true; break; }
+                } else {
+                    M = fmaxf(M, v);
+                }
             }
         }
-        if (counters) atomicAdd(counters, count);
+        if (counters) { atomicAdd(counters, visited); atomicAdd(counters + 1, evaluated); }
     } else {
-        // Row-cached sampler (sampler.cuh); the blend of sample j-1 is issued after the loads of sample j
-        // so that classification and blending overlap the load latency.
+        // Row-cached sampler (sampler.cuh); the blend of the previous evaluated sample is issued after the loads
+        // of the current one so that classification and blending overlap the load latency.
         RowCache K;
         cache_init(K);
         const unsigned long long vol_base = reinterpret_cast<unsigned long long>(vol);
         const unsigned slab_bytes = P.slab_stride * 4u;
-        float vprev = sample_cached(vol_base, P.ty_stride, slab_bytes, nxm1, nym1, nzm1, q0x, q0y, q0z, K);
-        bool done = false;
-#ifdef VR_EXP_L2PREFETCH
-        // EXPERIMENT (rejected, profiles/r02_experiments.md; build with VR_DEFINES=-DVR_EXP_L2PREFETCH, run with
-        // VR_PF=every,ahead): L2 tile prefetch.  Every pf_every samples the ray looks pf_ahead samples ahead and, when
-        // that point lies in an 8^3 tile it has not asked for yet, has the bulk-copy engine pull the whole 2 KB
-        // tile into the L2 (cp.async.bulk.prefetch.L2: one request per tile instead of one per 32-byte sector,
-        // and the row loads that follow find L2 latency instead of HBM latency).  Lanes of the warp that want the same
-        // tile are merged with match.any.  Purely a hint: no effect on any value.
-        unsigned pf_last = 0xffffffffu;
-        const unsigned pf_mask = (unsigned)P.pf_every - 1u;
-        const unsigned tiles_row = P.ty_stride >> 9, tiles_slab = P.slab_stride >> 9;
-#endif
-        for (int j = 1; j < n; ++j) {
-#ifdef VR_EXP_L2PREFETCH
-            if (P.pf_every && ((unsigned)j & pf_mask) == 0u && j + P.pf_ahead < n) {
-                const float ja = (float)(j + P.pf_ahead);
-                const float ax = fminf(fmaxf(fmaf(ja, hx, q0x), 0.0f), nxm1), ay = fminf(fmaxf(fmaf(ja, hy, q0y), 0.0f), nym1),
-                            az = fminf(fmaxf(fmaf(ja, hz, q0z), 0.0f), nzm1);
-                const unsigned tid = ((unsigned)az >> 3) * tiles_slab + ((unsigned)ay >> 3) * tiles_row + ((unsigned)ax >> 3);
-                if (tid != pf_last) {
-                    pf_last = tid;
-                    const unsigned peers = __match_any_sync(__activemask(), tid);
-                    if ((peers & ((1u << (threadIdx.x & 31)) - 1u)) == 0u) {
-                        const unsigned long long a = vol_base + (unsigned long long)tid * (TILE_ELEMS * 4ull);
-                        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(a), "r"(TILE_ELEMS * 4) : "memory");
+        float vprev = 0.f;
+        bool have = false, done = false;
+        for (int js = 0; js < n && !done; js += P.seg_len) {
+            Anchor An;
+            set_anchor(o, d, t_near, P.step, i_lo + js, h, P.seg_span, An);
+            const int je = min(n - js, P.seg_len);
+            if (SKIP) {
+                unsigned todo_lo = 0u, todo_hi = 0u;          // bit jl: sample jl of this segment can contribute
+                for (int jl = 0; jl < je; ++jl) {
+                    unsigned ix, iy, iz;
+                    locate_cell(An, jl, h, ix, iy, iz);
+                    const unsigned occ = cell_occupied(mask, nbx, nbxy, ix, iy, iz, mc) ? 1u : 0u;
+                    if (jl < 32) todo_lo |= occ << jl; else todo_hi |= occ << (jl - 32);
+                }
+                while (todo_lo | todo_hi) {
+                    int jl;
+                    if (todo_lo) { jl = __ffs((int)todo_lo) - 1; todo_lo &= todo_lo - 1u; }
+                    else { jl = 31 + __ffs((int)todo_hi); todo_hi &= todo_hi - 1u; }
+                    Cell c;
+                    locate(An, jl, h, c);
+                    const float v = sample_cached(vol_base, P.ty_stride, slab_bytes, c, K);
+                    if (have) {
+                        classify_blend(tf, P, vprev, Cr, Cg, Cb, A);
+                        if (P.ert_on && A >= P.ert) { done = true; break; }
                     }
+                    vprev = v; have = true;
+                }
+            } else {
+                for (int jl = 0; jl < je; ++jl) {
+                    Cell c;
+                    locate(An, jl, h, c);
+                    const float v = sample_cached(vol_base, P.ty_stride, slab_bytes, c, K);
+                    if (have) {
+                        if (MODE == MODE_EA) {
+                            classify_blend(tf, P, vprev, Cr, Cg, Cb, A);
+                            if (P.ert_on && A >= P.ert) { done = true; break; }
+                        } else {
+                            M = fmaxf(M, vprev);
+                        }
+                    }
+                    vprev = v; have = true;
                 }
             }
-#endif
-            const float jf = (float)j;
-            const float v = sample_cached(vol_base, P.ty_stride, slab_bytes, nxm1, nym1, nzm1,
-                                          fmaf(jf, hx, fmaf(jf, ex, q0x)), fmaf(jf, hy, fmaf(jf, ey, q0y)),
-                                          fmaf(jf, hz, fmaf(jf, ez, q0z)), K);
-            if (MODE == MODE_EA) {
-                classify_blend(tf, P, vprev, Cr, Cg, Cb, A);
-                if (P.ert_on && A >= P.ert) { done = true; break; }
-            } else {
-                M = fmaxf(M, vprev);
-            }
-            vprev = v;
         }
-        if (!done) {
+        if (have && !done) {
             if (MODE == MODE_EA) classify_blend(tf, P, vprev, Cr, Cg, Cb, A);
             else M = fmaxf(M, vprev);
         }

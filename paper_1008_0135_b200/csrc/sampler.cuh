@@ -1,7 +1,16 @@
-// sampler.cuh — O5 trilinear sampling of the tiled cube with a per-ray register cache of x-rows.
+// sampler.cuh — O5 trilinear sampling of the tiled cube: segment-anchored positions, a per-ray register
+// cache of x-rows, and the occupancy-mask test of empty-space skipping.
 //
-// ncu of the first caster (profiles/r01_cast_full.md) showed the L1TEX data stage at 96 %: eight scalar
-// corner loads per sample, each a warp request over ~20-32 distinct lines.  Here a ray keeps, in
+// Positions.  A ray's samples are t_i = t_near + (i + 1/2) step (O4).  Absolute fp32 coordinates reach 2048
+// on the headline cube, where half an ulp is 6e-5 voxel: against noise with voxel-to-voxel differences of
+// several units that is ~3e-4 in the interpolated value — inside the 1e-4 RGBA gate (each sample carries a
+// small alpha) but not inside the 1e-4 gate on raw MIP maxima.  So the march is cut into SEGMENTS of
+// P.seg_len samples; at the start of a segment the position is evaluated in double (the oracle's expression),
+// split into an integer origin O and a remainder rel in [0, seg span], and inside the segment
+// q_rel(j') = rel + j' h in fp32 with |q_rel| <= ~65: rounding <= 4e-6 voxel.  Voxel index = O + floor(q_rel).
+//
+// Row cache.  ncu of the first caster (profiles/r01cd_cast_full.md) showed the L1TEX data stage at 96 %: eight
+// scalar corner loads per sample, each a warp request over ~20-32 distinct lines.  Here a ray keeps, in
 // registers, the four 16-byte x-chunks (4 voxels each) that hold its current 2x2 (y,z) rows and loads a
 // row only when the ray has moved off it:
 //   * x0 and x0+1 come out of ONE 128-bit load per row (plus one scalar load only when x0 is the last
@@ -10,7 +19,7 @@
 //     axis always have different parity, and when the ray advances by one voxel the row it keeps stays in
 //     its slot while the new row replaces the one left behind — no data movement, no dependence on the
 //     direction of travel, and any step length is handled (a slot is reloaded whenever the row index it
-//     should hold differs from the one it holds).
+//     should hold differs from the one it holds), including the jumps empty-space skipping makes.
 // Values and weights are those of O5 exactly (same voxels, same fractions).
 #pragma once
 #include <cuda_runtime.h>
@@ -48,20 +57,83 @@ __device__ __forceinline__ const float* elem_ptr(unsigned long long base, unsign
     return reinterpret_cast<const float*>(a);
 }
 
-// Returns the trilinear value at (qx,qy,qz) = position - 1/2.
+// Segment anchor: integer origin and remainder of the segment's first sample, in PADDED coordinates
+// u = q + 1 = p + 1/2 (kernels.cuh, re-layout): no clamp is needed, the replicated layers do O5's clamp-to-edge.
+struct Anchor {
+    int O[3];
+    float rel[3];
+};
+
+// Anchor of the segment whose first sample has lattice index i0 (double precision; O2-O4's expressions).
+// span >= seg_len * |h_a| + 1 is subtracted on axes the ray descends, so that u_rel stays non-negative over
+// the whole segment (the magic-add floor below needs that).
+__device__ __forceinline__ void set_anchor(const double o[3], const double d[3], double t_near, double step,
+                                           long long i0, const float h[3], int span, Anchor& A) {
+    const double ta = t_near + ((double)i0 + 0.5) * step;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double ud = o[a] + ta * d[a] + 0.5;
+        const double base = floor(ud) - (h[a] < 0.0f ? (double)span : 0.0);
+        A.O[a] = (int)base;
+        A.rel[a] = (float)(ud - base);
+    }
+}
+
+struct Cell {                // padded cell of one sample: low corner and fractions
+    unsigned ix, iy, iz;
+    float fx, fy, fz;
+};
+
+// Sample jl of the segment: u_rel = rel + jl h, floor by the 2^23 magic add (no F2I/I2F), index = O + floor.
+__device__ __forceinline__ void locate(const Anchor& A, int jl, const float h[3], Cell& c) {
+    const float jf = (float)jl;
+    float q[3], r[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        q[a] = fmaf(jf, h[a], A.rel[a]);
+        r[a] = __fadd_rd(q[a], 8388608.0f);       // 0 <= q < 2^22: the integer is the low mantissa bits
+    }
+    c.ix = (unsigned)(A.O[0] + (int)(__float_as_uint(r[0]) & 0x7fffffu));
+    c.iy = (unsigned)(A.O[1] + (int)(__float_as_uint(r[1]) & 0x7fffffu));
+    c.iz = (unsigned)(A.O[2] + (int)(__float_as_uint(r[2]) & 0x7fffffu));
+    c.fx = q[0] - (r[0] - 8388608.0f);
+    c.fy = q[1] - (r[1] - 8388608.0f);
+    c.fz = q[2] - (r[2] - 8388608.0f);
+}
+
+// The same cell without the fractions (occupancy pass of empty-space skipping).
+__device__ __forceinline__ void locate_cell(const Anchor& A, int jl, const float h[3], unsigned& ix, unsigned& iy,
+                                            unsigned& iz) {
+    const float jf = (float)jl;
+    ix = (unsigned)(A.O[0] + (int)(__float_as_uint(__fadd_rd(fmaf(jf, h[0], A.rel[0]), 8388608.0f)) & 0x7fffffu));
+    iy = (unsigned)(A.O[1] + (int)(__float_as_uint(__fadd_rd(fmaf(jf, h[1], A.rel[1]), 8388608.0f)) & 0x7fffffu));
+    iz = (unsigned)(A.O[2] + (int)(__float_as_uint(__fadd_rd(fmaf(jf, h[2], A.rel[2]), 8388608.0f)) & 0x7fffffu));
+}
+
+// Empty-space skipping (NEXT-2): one bit per padded cell, set when a sample inside the cell can be non-transparent
+// (build_mask_kernel).  Words of 64 bits = 4x4x4 cells, word index ((bz*NBY + by)*NBX + bx); the ray keeps the
+// word of its current block in registers and reloads it only when it enters another block.
+struct MaskCursor {
+    unsigned lo, hi;         // the 64-bit word: lo = cells with (iz & 3) < 2
+    unsigned tag;
+};
+__device__ __forceinline__ bool cell_occupied(const unsigned long long* __restrict__ mask, unsigned nbx, unsigned nbxy,
+                                              unsigned ix, unsigned iy, unsigned iz, MaskCursor& mc) {
+    const unsigned tag = (iz >> 2) * nbxy + (iy >> 2) * nbx + (ix >> 2);
+    if (tag != mc.tag) {
+        const uint2 w = __ldg(reinterpret_cast<const uint2*>(mask + tag));
+        mc.lo = w.x; mc.hi = w.y; mc.tag = tag;
+    }
+    const unsigned half = (iz & 2u) ? mc.hi : mc.lo;
+    const unsigned bit = ((iz & 1u) << 4) | ((iy & 3u) << 2) | (ix & 3u);
+    return (half >> bit) & 1u;
+}
+
+// Trilinear value of the cell (O5) through the row cache.
 // vol_base: address of the tiled cube; ty_stride in elements; slab_bytes = bytes between z-tile slabs.
 __device__ __forceinline__ float sample_cached(unsigned long long vol_base, unsigned ty_stride, unsigned slab_bytes,
-                                               float nxm1, float nym1, float nzm1, float qx, float qy, float qz,
-                                               RowCache& K) {
-    qx = fminf(fmaxf(qx, 0.0f), nxm1);
-    qy = fminf(fmaxf(qy, 0.0f), nym1);
-    qz = fminf(fmaxf(qz, 0.0f), nzm1);
-    // floor of a non-negative float < 2^22 without F2I/I2F: add 2^23 rounding down; the integer is the low
-    // mantissa bits and (r - 2^23) is that integer as a float, exactly.
-    const float rx = __fadd_rd(qx, 8388608.0f), ry = __fadd_rd(qy, 8388608.0f), rz = __fadd_rd(qz, 8388608.0f);
-    const unsigned ix = __float_as_uint(rx) & 0x7fffffu, iy = __float_as_uint(ry) & 0x7fffffu,
-                   iz = __float_as_uint(rz) & 0x7fffffu;
-    const float fx = qx - (rx - 8388608.0f), fy = qy - (ry - 8388608.0f), fz = qz - (rz - 8388608.0f);
+                                               const Cell& s, RowCache& K) {
+    const unsigned ix = s.ix, iy = s.iy, iz = s.iz;
     const unsigned cx = ix >> 2, c = ix & 3;
     const bool straddle = (c == 3);
 
@@ -74,30 +146,36 @@ __device__ __forceinline__ float sample_cached(unsigned long long vol_base, unsi
     const bool e_all = !K.straddle;
 
     const unsigned exc = (cx >> 1) * TILE_ELEMS + ((cx & 1) << 2);
-    const unsigned ix1 = ix + 1;
-    const unsigned exe = (ix1 >> 3) * TILE_ELEMS + (ix1 & 7);
     const unsigned ey[2] = {(wy[0] >> 3) * ty_stride + ((wy[0] & 7) << 3),
                             (wy[1] >> 3) * ty_stride + ((wy[1] & 7) << 3)};
-    unsigned long long pz[2];
-    unsigned ez[2];
+    // Row addresses are formed ONCE, unconditionally (volatile: ptxas otherwise re-derives the whole offset inside
+    // each predicated load, +80 instructions per sample); the loads themselves stay predicated.
+    unsigned long long rp[2][2];
 #pragma unroll
     for (int b = 0; b < 2; ++b) {
-        asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(pz[b]) : "r"(wz[b] >> 3), "r"(slab_bytes), "l"(vol_base));
-        ez[b] = (wz[b] & 7) << 6;
+        unsigned long long pz;
+        asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(pz) : "r"(wz[b] >> 3), "r"(slab_bytes), "l"(vol_base));
+        const unsigned ez = ((wz[b] & 7) << 6) + exc;
+#pragma unroll
+        for (int a = 0; a < 2; ++a)
+            asm volatile("mad.wide.u32 %0, %1, 4, %2;" : "=l"(rp[a][b]) : "r"(ez + ey[a]), "l"(pz));
     }
+    // byte distance from the chunk to voxel ix + 1 when ix is the chunk's last voxel: the next chunk of the same tile
+    // row (16 B on) or, from a tile's second chunk, the first voxel of the next tile in x ((512 - 4) * 4 B on)
+    const unsigned de = (ix & 4u) ? (TILE_ELEMS - 4) * 4u : 16u;
 #pragma unroll
     for (int a = 0; a < 2; ++a)
 #pragma unroll
         for (int b = 0; b < 2; ++b) {
             const bool need = xchg || ychg[a] || zchg[b];
-            if (need) K.r[a][b] = __ldg(reinterpret_cast<const float4*>(elem_ptr(pz[b], exc + ey[a] + ez[b])));
-            if (straddle && (need || e_all)) K.e[a][b] = __ldg(elem_ptr(pz[b], exe + ey[a] + ez[b]));
+            if (need) K.r[a][b] = __ldg(reinterpret_cast<const float4*>(rp[a][b]));
+            if (straddle && (need || e_all)) K.e[a][b] = __ldg(reinterpret_cast<const float*>(rp[a][b] + de));
         }
     K.cx = cx; K.hy[0] = wy[0]; K.hy[1] = wy[1]; K.hz[0] = wz[0]; K.hz[1] = wz[1]; K.straddle = straddle;
 
     // O5 blend: x inside each row, then y, then z.  Slot 0 holds the even row: it is row i when i is even
     // (weight 1-f) and row i+1 when i is odd (weight f).
-    const float gy = (iy & 1) ? 1.0f - fy : fy, gz = (iz & 1) ? 1.0f - fz : fz;
+    const float gy = (iy & 1) ? 1.0f - s.fy : s.fy, gz = (iz & 1) ? 1.0f - s.fz : s.fz;
     float row[2][2];
 #pragma unroll
     for (int a = 0; a < 2; ++a)
@@ -105,7 +183,7 @@ __device__ __forceinline__ float sample_cached(unsigned long long vol_base, unsi
         for (int b = 0; b < 2; ++b) {
             const float v0 = pick4(K.r[a][b], c, 0.0f);
             const float v1 = pick4(K.r[a][b], c + 1, K.e[a][b]);
-            row[a][b] = fmaf(fx, v1 - v0, v0);
+            row[a][b] = fmaf(s.fx, v1 - v0, v0);
         }
     const float c0 = fmaf(gy, row[1][0] - row[0][0], row[0][0]);
     const float c1 = fmaf(gy, row[1][1] - row[0][1], row[0][1]);

@@ -63,7 +63,16 @@ struct vr_volume {
     float* d_frame = nullptr;         // internal frame of vr_render_to_host
     size_t frame_floats = 0;
 
-    int pf_every = 0, pf_ahead = 0;   // L2 tile prefetch of the caster (0 = off); env VR_PF="every,ahead" overrides
+    // NEXT-2 empty-space skipping: occupancy mask (one bit per voxel cell), built for the current table on demand
+    bool skip_enabled = true;
+    unsigned long long* d_mask = nullptr;
+    unsigned long long* d_mask_count = nullptr;
+    int NBX = 0, NBY = 0, NBZ = 0;
+    size_t mask_words = 0;
+    bool mask_valid = false;
+    float mask_key[3] = {0.f, 0.f, 0.f};   // vmin, inv_range, x_zero_below the mask was built for
+    float mask_build_ms = 0.f;
+    long long mask_occupied = 0;
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};   // cast begin/end, composite begin/end
     bool timed_cast = false, timed_comp = false;
 };
@@ -92,6 +101,19 @@ vr_status check_render_args(const vr_volume* vol, const vr_camera* cam, int W, i
     return VR_OK;
 }
 
+// x_zero_below of the current table: (index of the first entry with alpha > 0) - 1
+float table_zero_below(const vr_volume* vol) {
+    int j0 = 0;
+    while (j0 < 256 && !(vol->tf_host[4 * j0 + 3] > 0.0f)) ++j0;
+    return (float)(j0 - 1);
+}
+
+// Empty-space skipping applies to emission-absorption frames whose table starts with at least two transparent
+// entries (otherwise no cell can be proven empty and the mask would be all ones).
+bool skip_applies(const vr_volume* vol, int mode) {
+    return vol->skip_enabled && mode == VR_MODE_EA && table_zero_below(vol) - vr::MASK_MARGIN > 0.0f;
+}
+
 // cropped = true: brick images are rect-sized and packed (vr_render); false: full W x H frames.
 vr_status build_frame(const vr_volume* vol, const vr_camera* cam, int W, int H, float step, float ert, bool cropped,
                       bool direct, Frame& f) {
@@ -112,12 +134,11 @@ vr_status build_frame(const vr_volume* vol, const vr_camera* cam, int W, int H, 
     P.inv_range = 1.0f / (vol->vmax - vol->vmin);
     P.ert_on = (ert > 0.0f && ert < 1.0f) ? 1 : 0;
     P.ert = ert;
-    P.pf_every = vol->pf_every; P.pf_ahead = vol->pf_ahead;
-    {   // first table entry with alpha > 0 (the per-step correction keeps zeros zero)
-        int j0 = 0;
-        while (j0 < 256 && !(vol->tf_host[4 * j0 + 3] > 0.0f)) ++j0;
-        P.x_zero_below = (float)(j0 - 1);
-    }
+    // segments of <= 64 voxels of path (sampler.cuh): fp32 positions stay within ~65 of their anchor
+    P.seg_len = std::max(1, std::min(64, (int)(64.0 / (double)step)));
+    P.seg_span = (int)std::ceil((double)P.seg_len * (double)step) + 1;
+    P.nbx = vol->NBX; P.nby = vol->NBY;
+    P.x_zero_below = table_zero_below(vol);   // the per-step opacity correction keeps zeros zero
 
     std::vector<vr::BrickPlan> plan;
     vr::plan_bricks(vol->dims, vol->bricks, *cam, W, H, plan, f.order, vol->sub_lo, vol->sub_hi);
@@ -184,17 +205,56 @@ vr_status upload_tf_for_step(vr_volume* vol, double step) {
     return VR_OK;
 }
 
+// Build (or reuse) the occupancy mask for the current table.  One pass over the tiled cube.
+vr_status ensure_mask(vr_volume* vol) {
+    const float key[3] = {vol->vmin, 1.0f / (vol->vmax - vol->vmin), table_zero_below(vol)};
+    if (vol->mask_valid && std::memcmp(key, vol->mask_key, sizeof(key)) == 0) return VR_OK;
+    if (!vol->d_mask) {
+        VR_CUDA(cudaMalloc(&vol->d_mask, vol->mask_words * sizeof(unsigned long long)), "allocate occupancy mask");
+        VR_CUDA(cudaMalloc(&vol->d_mask_count, sizeof(unsigned long long)), "allocate occupancy counter");
+    }
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    VR_CUDA(cudaEventCreate(&e0), "create event");
+    cudaError_t e = cudaEventCreate(&e1);
+    if (e == cudaSuccess) e = cudaMemsetAsync(vol->d_mask_count, 0, sizeof(unsigned long long), vol->stream);
+    if (e == cudaSuccess) e = cudaEventRecord(e0, vol->stream);
+    if (e == cudaSuccess) {
+        dim3 grid((vol->dims[0] + 1 + 31) / 32, (vol->dims[1] + 1 + 7) / 8, (vol->dims[2] + 1 + 7) / 8);
+        vr::build_mask_kernel<<<grid, 256, 0, vol->stream>>>(
+            vol->d_tiled, (unsigned)vol->TX * vr::TILE_ELEMS, (unsigned)vol->TX * (unsigned)vol->TY * vr::TILE_ELEMS,
+            vol->dims[0], vol->dims[1], vol->dims[2], key[0], key[1], key[2], vol->d_mask, vol->NBX, vol->NBY,
+            vol->d_mask_count);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaEventRecord(e1, vol->stream);
+    unsigned long long cnt = 0;
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&cnt, vol->d_mask_count, sizeof(cnt), cudaMemcpyDeviceToHost, vol->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(vol->stream);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&vol->mask_build_ms, e0, e1);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (e != cudaSuccess) return cuda_fail(e, "build occupancy mask");
+    vol->mask_occupied = (long long)cnt;
+    std::memcpy(vol->mask_key, key, sizeof(key));
+    vol->mask_valid = true;
+    return VR_OK;
+}
+
 template <int INSTR>
 vr_status launch_cast(vr_volume* vol, const Frame& f, int mode, float* d_img, unsigned long long* d_counter,
-                      unsigned* d_bitmap) {
+                      unsigned* d_bitmap, unsigned* d_mask_bitmap) {
     if (f.total_tiles == 0) return VR_OK;
     const int B = (int)f.recs.size();
-    if (mode == VR_MODE_EA)
-        vr::cast_kernel<vr::MODE_EA, INSTR><<<f.total_tiles, vr::CTA_THREADS, 0, vol->stream>>>(
-            f.P, vol->d_bricks, B, vol->d_tiled, vol->d_tf_ea, d_img, d_counter, d_bitmap);
-    else
-        vr::cast_kernel<vr::MODE_MIP, INSTR><<<f.total_tiles, vr::CTA_THREADS, 0, vol->stream>>>(
-            f.P, vol->d_bricks, B, vol->d_tiled, vol->d_tf_ea, d_img, d_counter, d_bitmap);
+    const bool skip = skip_applies(vol, mode) && vol->mask_valid;     // callers run ensure_mask first
+#define VR_LAUNCH(MODE_, SKIP_)                                                                              \
+    vr::cast_kernel<MODE_, INSTR, SKIP_><<<f.total_tiles, vr::CTA_THREADS, 0, vol->stream>>>(                \
+        f.P, vol->d_bricks, B, vol->d_tiled, vol->d_tf_ea, vol->d_mask, d_img, d_counter, d_bitmap, d_mask_bitmap)
+    if (mode == VR_MODE_EA) {
+        if (skip) VR_LAUNCH(vr::MODE_EA, 1); else VR_LAUNCH(vr::MODE_EA, 0);
+    } else {
+        VR_LAUNCH(vr::MODE_MIP, 0);
+    }
+#undef VR_LAUNCH
     VR_CUDA(cudaGetLastError(), "cast kernel launch");
     return VR_OK;
 }
@@ -236,18 +296,14 @@ vr_status vr_create_volume(const int dims[3], const float* d_data, vr_volume** o
     vr_volume* v = new (std::nothrow) vr_volume();
     if (!v) return fail(VR_ERR_OOM, "vr_create_volume: host allocation failed");
     for (int a = 0; a < 3; ++a) { v->dims[a] = dims[a]; v->sub_hi[a] = dims[a]; }
-    if (const char* pf = std::getenv("VR_PF")) {           // tuning knob, see DESIGN.md "Kernels"
-        int ev_ = 0, ah = 0;
-        if (std::sscanf(pf, "%d,%d", &ev_, &ah) == 2 && ev_ >= 0 && ev_ <= 64 && (ev_ & (ev_ - 1)) == 0 && ah >= 0 && ah <= 256) {
-            v->pf_every = ev_; v->pf_ahead = ah;
-        }
-    }
-    v->TX = (dims[0] + 1 + 7) / 8; v->TY = (dims[1] + 1 + 7) / 8; v->TZ = (dims[2] + 1 + 7) / 8;
+    v->TX = (dims[0] + 2 + 7) / 8; v->TY = (dims[1] + 2 + 7) / 8; v->TZ = (dims[2] + 2 + 7) / 8;   // padded: +1 layer each side
     if ((double)v->TX * v->TY * vr::TILE_ELEMS >= 1073741824.0) {   // slab bytes and in-slab offsets stay 32-bit
         delete v;
         return fail(VR_ERR_INVALID_ARG, "vr_create_volume: nx*ny too large for 32-bit in-slab offsets");
     }
     v->tiled_elems = (size_t)v->TX * v->TY * v->TZ * vr::TILE_ELEMS;
+    v->NBX = (dims[0] + 1 + 3) / 4; v->NBY = (dims[1] + 1 + 3) / 4; v->NBZ = (dims[2] + 1 + 3) / 4;   // n_a + 1 padded cells
+    v->mask_words = (size_t)v->NBX * v->NBY * v->NBZ;
     cudaError_t e = cudaMalloc(&v->d_tiled, v->tiled_elems * sizeof(float));
     if (e == cudaSuccess) e = cudaMalloc(&v->d_range, 2 * vr::RANGE_SLOTS * sizeof(unsigned));
     if (e == cudaSuccess) e = cudaMalloc(&v->d_tf_ea, 256 * sizeof(float4));
@@ -305,6 +361,8 @@ void vr_destroy_volume(vr_volume* v) {
     if (v->d_order) cudaFree(v->d_order);
     if (v->d_pool) cudaFree(v->d_pool);
     if (v->d_frame) cudaFree(v->d_frame);
+    if (v->d_mask) cudaFree(v->d_mask);
+    if (v->d_mask_count) cudaFree(v->d_mask_count);
     for (int k = 0; k < 4; ++k)
         if (v->ev[k]) cudaEventDestroy(v->ev[k]);
     delete v;
@@ -369,8 +427,9 @@ vr_status vr_render(vr_volume* vol, const vr_camera* cam, int W, int H, float st
     if (mode == VR_MODE_EA && (s = upload_tf_for_step(vol, (double)step)) != VR_OK) return s;
     vol->timed_cast = vol->timed_comp = false;
     if (!direct && (s = ensure_pool(vol, f.pool_pixels * (mode == VR_MODE_EA ? 4 : 1))) != VR_OK) return s;
+    if (skip_applies(vol, mode) && (s = ensure_mask(vol)) != VR_OK) return s;   // builds only after a table change
     VR_CUDA(cudaEventRecord(vol->ev[0], vol->stream), "record event");
-    s = launch_cast<0>(vol, f, mode, direct ? d_out_rgba : vol->d_pool, nullptr, nullptr);
+    s = launch_cast<0>(vol, f, mode, direct ? d_out_rgba : vol->d_pool, nullptr, nullptr, nullptr);
     if (s != VR_OK) return s;
     VR_CUDA(cudaEventRecord(vol->ev[1], vol->stream), "record event");
     vol->timed_cast = true;
@@ -428,7 +487,8 @@ vr_status vr_render_bricks(vr_volume* vol, const vr_camera* cam, int W, int H, f
     const size_t n = B * (size_t)W * H * (mode == VR_MODE_EA ? 4 : 1);
     vr::fill_kernel<<<1184, 256, 0, vol->stream>>>(d_brick_images, n, mode == VR_MODE_EA ? 0.0f : -INFINITY);
     VR_CUDA(cudaGetLastError(), "fill kernel launch");
-    return launch_cast<0>(vol, f, mode, d_brick_images, nullptr, nullptr);
+    if (skip_applies(vol, mode) && (s = ensure_mask(vol)) != VR_OK) return s;
+    return launch_cast<0>(vol, f, mode, d_brick_images, nullptr, nullptr, nullptr);
 }
 
 vr_status vr_composite(vr_volume* vol, const vr_camera* cam, int W, int H, int mode, const float* d_brick_images,
@@ -465,8 +525,8 @@ vr_status vr_plan_bricks(const int dims[3], const int bricks[3], const vr_camera
     return VR_OK;
 }
 
-static vr_status measure_impl(vr_volume* vol, const vr_camera* cam, int W, int H, float step, int mode, float ert,
-                              long long* h_samples, long long h_units[3]) {
+vr_status vr_measure_units(vr_volume* vol, const vr_camera* cam, int W, int H, float step, int mode, float ert,
+                           long long h_samples[2], long long h_units[4]) {
     vr_status s = check_render_args(vol, cam, W, H, step, mode);
     if (s != VR_OK) return s;
     Frame f;
@@ -474,44 +534,66 @@ static vr_status measure_impl(vr_volume* vol, const vr_camera* cam, int W, int H
     if ((s = upload_plan(vol, f)) != VR_OK) return s;
     if (mode == VR_MODE_EA && (s = upload_tf_for_step(vol, (double)step)) != VR_OK) return s;
     if ((s = ensure_pool(vol, f.pool_pixels * (mode == VR_MODE_EA ? 4 : 1))) != VR_OK) return s;
+    if (skip_applies(vol, mode) && (s = ensure_mask(vol)) != VR_OK) return s;
     const size_t n_words = (vol->tiled_elems / 8 + 31) / 32;
-    unsigned* d_bitmap = nullptr;
-    unsigned long long* d_cnt = nullptr;
-    VR_CUDA(cudaMalloc(&d_bitmap, n_words * sizeof(unsigned)), "allocate sector bitmap");
-    cudaError_t e = cudaMalloc(&d_cnt, 4 * sizeof(unsigned long long));
-    if (e != cudaSuccess) { cudaFree(d_bitmap); return cuda_fail(e, "allocate counters"); }
-    e = cudaMemsetAsync(d_bitmap, 0, n_words * sizeof(unsigned), vol->stream);
-    if (e == cudaSuccess) e = cudaMemsetAsync(d_cnt, 0, 4 * sizeof(unsigned long long), vol->stream);
-    if (e != cudaSuccess) s = cuda_fail(e, "vr_measure: clear counters");
-    if (s == VR_OK) s = launch_cast<1>(vol, f, mode, vol->d_pool, d_cnt, d_bitmap);
-    unsigned long long h[4] = {0, 0, 0, 0};
+    const size_t m_words = (vol->mask_words / 4 + 31) / 32 + 1;      // one bit per 32-byte sector (4 words) of the mask
+    unsigned *d_bitmap = nullptr, *d_mbitmap = nullptr;
+    unsigned long long* d_cnt = nullptr;                              // [0..1] samples, [2..4] cube units, [5..7] mask units
+    cudaError_t e = cudaMalloc(&d_bitmap, n_words * sizeof(unsigned));
+    if (e == cudaSuccess) e = cudaMalloc(&d_mbitmap, m_words * sizeof(unsigned));
+    if (e == cudaSuccess) e = cudaMalloc(&d_cnt, 8 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemsetAsync(d_bitmap, 0, n_words * sizeof(unsigned), vol->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(d_mbitmap, 0, m_words * sizeof(unsigned), vol->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(d_cnt, 0, 8 * sizeof(unsigned long long), vol->stream);
+    if (e != cudaSuccess) s = cuda_fail(e, "vr_measure: allocate / clear counters");
+    if (s == VR_OK) s = launch_cast<1>(vol, f, mode, vol->d_pool, d_cnt, d_bitmap, d_mbitmap);
+    unsigned long long h[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     if (s == VR_OK) {
-        vr::popcount_kernel<<<1184, 256, 0, vol->stream>>>(d_bitmap, n_words, d_cnt + 1);
+        vr::popcount_kernel<<<1184, 256, 0, vol->stream>>>(d_bitmap, n_words, d_cnt + 2);
+        vr::popcount_kernel<<<148, 256, 0, vol->stream>>>(d_mbitmap, m_words, d_cnt + 5);
         e = cudaGetLastError();
         if (e == cudaSuccess) e = cudaMemcpyAsync(h, d_cnt, sizeof(h), cudaMemcpyDeviceToHost, vol->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(vol->stream);
         if (e != cudaSuccess) s = cuda_fail(e, "vr_measure");
     }
-    cudaFree(d_bitmap);
-    cudaFree(d_cnt);
+    if (d_bitmap) cudaFree(d_bitmap);
+    if (d_mbitmap) cudaFree(d_mbitmap);
+    if (d_cnt) cudaFree(d_cnt);
     if (s != VR_OK) return s;
-    if (h_samples) *h_samples = (long long)h[0];
-    if (h_units) for (int k = 0; k < 3; ++k) h_units[k] = (long long)h[1 + k];
+    if (h_samples) { h_samples[0] = (long long)h[0]; h_samples[1] = (long long)h[1]; }
+    if (h_units) { for (int k = 0; k < 3; ++k) h_units[k] = (long long)h[2 + k]; h_units[3] = (long long)h[5]; }
     return VR_OK;
 }
 
 vr_status vr_measure(vr_volume* vol, const vr_camera* cam, int W, int H, float step, int mode, float ert,
                      long long* h_samples, long long* h_sectors) {
-    long long u[3] = {0, 0, 0};
-    vr_status s = measure_impl(vol, cam, W, H, step, mode, ert, h_samples, u);
+    long long c[2] = {0, 0}, u[4] = {0, 0, 0, 0};
+    vr_status s = vr_measure_units(vol, cam, W, H, step, mode, ert, c, u);
+    if (s == VR_OK && h_samples) *h_samples = c[0];
     if (s == VR_OK && h_sectors) *h_sectors = u[0];
     return s;
 }
 
-vr_status vr_measure_units(vr_volume* vol, const vr_camera* cam, int W, int H, float step, int mode, float ert,
-                           long long* h_samples, long long h_units[3]) {
-    if (!h_units) return fail(VR_ERR_INVALID_ARG, "vr_measure_units: h_units is NULL");
-    return measure_impl(vol, cam, W, H, step, mode, ert, h_samples, h_units);
+vr_status vr_set_empty_space_skipping(vr_volume* vol, int enabled) {
+    if (!vol) return fail(VR_ERR_INVALID_ARG, "vr_set_empty_space_skipping: volume is NULL");
+    vol->skip_enabled = enabled != 0;
+    return VR_OK;
+}
+
+vr_status vr_get_skip_info(vr_volume* vol, int* h_active, float* h_build_ms, long long* h_mask_bytes,
+                           double* h_occupied_fraction) {
+    if (!vol) return fail(VR_ERR_INVALID_ARG, "vr_get_skip_info: volume is NULL");
+    const bool active = vol->has_tf && skip_applies(vol, VR_MODE_EA);
+    if (active) {
+        vr_status s = ensure_mask(vol);
+        if (s != VR_OK) return s;
+    }
+    if (h_active) *h_active = active ? 1 : 0;
+    if (h_build_ms) *h_build_ms = active ? vol->mask_build_ms : 0.f;
+    if (h_mask_bytes) *h_mask_bytes = active ? (long long)(vol->mask_words * sizeof(unsigned long long)) : 0;
+    if (h_occupied_fraction)
+        *h_occupied_fraction = active ? (double)vol->mask_occupied / ((double)vol->dims[0] * vol->dims[1] * vol->dims[2]) : 1.0;
+    return VR_OK;
 }
 
 vr_status vr_set_l2_fetch_granularity(int bytes) {

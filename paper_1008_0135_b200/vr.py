@@ -19,7 +19,8 @@ VR_MAX_BRICKS = 512
 
 SYMBOLS = ["vr_create_volume", "vr_destroy_volume", "vr_set_stream", "vr_set_transfer_function",
            "vr_set_bricks", "vr_set_subcube", "vr_render", "vr_render_to_host", "vr_render_bricks", "vr_composite",
-           "vr_plan_bricks", "vr_measure", "vr_measure_units", "vr_set_l2_fetch_granularity",
+           "vr_plan_bricks", "vr_measure", "vr_measure_units", "vr_set_empty_space_skipping", "vr_get_skip_info",
+           "vr_set_l2_fetch_granularity",
            "vr_get_l2_fetch_granularity", "vr_get_stage_ms", "vr_volume_info", "vr_volume_range", "vr_export_linear", "vr_last_error"]
 
 
@@ -63,6 +64,8 @@ def lib():
                                  C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
         L.vr_measure_units.argtypes = [vp, cam, C.c_int, C.c_int, C.c_float, C.c_int, C.c_float,
                                        C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
+        L.vr_set_empty_space_skipping.argtypes = [vp, C.c_int]
+        L.vr_get_skip_info.argtypes = [vp, ip, fp, C.POINTER(C.c_longlong), C.POINTER(C.c_double)]
         L.vr_set_l2_fetch_granularity.argtypes = [C.c_int]
         L.vr_get_l2_fetch_granularity.argtypes = [ip]
         L.vr_get_stage_ms.argtypes = [vp, fp, fp]
@@ -215,18 +218,28 @@ class Volume:
         return out
 
     def vr_measure(self, cam, W, H, step, mode, ert_alpha=0.0):
-        """(samples evaluated, distinct 32-byte sectors touched) from the instrumented caster."""
+        """(lattice samples visited, distinct 32-byte sectors of the cube touched) from the instrumented caster."""
         s, k = C.c_longlong(0), C.c_longlong(0)
         _check(lib().vr_measure(self._h, C.byref(cam), int(W), int(H), float(step), int(mode),
                                 float(ert_alpha), C.byref(s), C.byref(k)))
         return s.value, k.value
 
     def vr_measure_units(self, cam, W, H, step, mode, ert_alpha=0.0):
-        """(samples evaluated, [distinct 32-byte sectors, 64-byte pairs, 128-byte lines] touched)."""
-        s, u = C.c_longlong(0), (C.c_longlong * 3)(0, 0, 0)
+        """([lattice samples visited, samples evaluated], [distinct 32-byte sectors, 64-byte pairs, 128-byte lines of
+        the cube touched, 32-byte sectors of the occupancy mask read])."""
+        s, u = (C.c_longlong * 2)(0, 0), (C.c_longlong * 4)(0, 0, 0, 0)
         _check(lib().vr_measure_units(self._h, C.byref(cam), int(W), int(H), float(step), int(mode),
-                                      float(ert_alpha), C.byref(s), u))
-        return s.value, [int(u[0]), int(u[1]), int(u[2])]
+                                      float(ert_alpha), s, u))
+        return [int(s[0]), int(s[1])], [int(u[k]) for k in range(4)]
+
+    def vr_set_empty_space_skipping(self, enabled):
+        _check(lib().vr_set_empty_space_skipping(self._h, 1 if enabled else 0))
+
+    def vr_get_skip_info(self):
+        """dict(active, build_ms, mask_bytes, occupied_fraction); builds the mask if it is due."""
+        a, ms, nb, fr = C.c_int(0), C.c_float(0), C.c_longlong(0), C.c_double(0)
+        _check(lib().vr_get_skip_info(self._h, C.byref(a), C.byref(ms), C.byref(nb), C.byref(fr)))
+        return {"active": bool(a.value), "build_ms": ms.value, "mask_bytes": nb.value, "occupied_fraction": fr.value}
 
     def vr_get_stage_ms(self):
         """(cast ms, composite ms) of the most recent vr_render; waits for it."""

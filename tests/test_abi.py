@@ -57,6 +57,8 @@ def test_null_and_range_checks_without_device(vr):
     assert L.vr_render_to_host(None, C.byref(cam), 8, 8, 1.0, 0, 0.0, None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_measure(None, C.byref(cam), 8, 8, 1.0, 0, 0.0, None, None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_measure_units(None, C.byref(cam), 8, 8, 1.0, 0, 0.0, None, None) == vr.VR_ERR_INVALID_ARG
+    assert L.vr_set_empty_space_skipping(None, 1) == vr.VR_ERR_INVALID_ARG
+    assert L.vr_get_skip_info(None, None, None, None, None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_set_l2_fetch_granularity(48) == vr.VR_ERR_INVALID_ARG
     assert L.vr_get_l2_fetch_granularity(None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_volume_info(None, None, None) == vr.VR_ERR_INVALID_ARG

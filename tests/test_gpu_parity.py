@@ -270,20 +270,21 @@ def test_measure_counts_every_sample_once(vr, oracle):
         vol.close()
         ref = oracle.render(cube.cpu().numpy(), tab, -3.0, 8.0, bricks, ocam(oracle, cs), W, H, 0.5, 0, 0.0, route=1)
         assert samples == ref["samples"]
-        total_sectors = -(-71 // 8) * -(-46 // 8) * -(-53 // 8) * 64
+        total_sectors = -(-72 // 8) * -(-47 // 8) * -(-54 // 8) * 64
         assert 0 < sectors <= total_sectors
 
 
 def _footprint_units(oracle, dims, cs, W, H, step, eps):
-    """Distinct 32/64/128-byte units of the tiled cube (8^3 tiles, T_a = ceil((n_a+1)/8),
-    element index ((tz*TY + ty)*TX + tx)*512 + lz*64 + ly*8 + lx, sector = index >> 3) touched by the 2x2x2
-    footprints (i0, i0+1 per axis, i0 = floor(clamp(p - 1/2, 0, n-1))) of the ORACLE's sample positions
+    """Distinct 32/64/128-byte units of the tiled cube (padded coordinates u = voxel + 1
+    with one replicated layer on each side, 8^3 tiles, T_a = ceil((n_a+2)/8), element index
+    ((tz*TY + ty)*TX + tx)*512 + lz*64 + ly*8 + lx of (ux,uy,uz), sector = index >> 3) touched by the 2x2x2
+    footprints (u0, u0+1 per axis, u0 = floor(p + 1/2)) of the ORACLE's sample positions
     t_i = t_near + (i + 1/2) step, enumerated here in numpy.  Returns (must, may): `must` counts only footprints
     whose floor is the same for any position error below eps voxels, `may` adds both candidates of the others —
     the GPU computes positions in fp32 (error ~1e-5 voxel at these sizes), so its count lies in [must, may]."""
     nx, ny, nz = dims
     n_a = np.array([nx, ny, nz])
-    TX, TY = (nx + 8) // 8, (ny + 8) // 8
+    TX, TY = (nx + 9) // 8, (ny + 9) // 8
     cam = oracle.make_camera(cs.view, cs.projection, cs.fovy_deg, cs.ortho_half_h)
     must, may = [], []
     for py in range(H):
@@ -293,11 +294,11 @@ def _footprint_units(oracle, dims, cs, W, H, step, eps):
             if n == 0:
                 continue
             t = tn + (np.arange(n) + 0.5) * step
-            q = np.clip(o[None, :] + t[:, None] * d[None, :] - 0.5, 0.0, (n_a - 1)[None, :])
+            q = o[None, :] + t[:, None] * d[None, :] + 0.5          # padded coordinates, in [1/2, n + 1/2]
             i0 = np.floor(q).astype(np.int64)
             f = q - i0
             lo_amb = (f < eps) & (i0 > 0)                       # could floor to i0 - 1
-            hi_amb = (f > 1.0 - eps) & (i0 < (n_a - 1)[None, :])  # could floor to i0 + 1
+            hi_amb = (f > 1.0 - eps) & (i0 < n_a[None, :])      # could floor to i0 + 1
             for shift, dest in ((0, must), (-1, None), (1, None)):
                 for corner in range(8):
                     c = np.array([(corner >> a) & 1 for a in range(3)])
@@ -320,8 +321,8 @@ def _footprint_units(oracle, dims, cs, W, H, step, eps):
     return units(must), units(may), must.size
 
 
-@pytest.mark.parametrize("proj,bricks,step,W,H", [(wl.PROJ_ORTHO, (1, 1, 1), 1.0, 40, 32), (wl.PROJ_PERSP, (2, 2, 2), 1.0, 36, 28),
-                                                  (wl.PROJ_ORTHO, (3, 1, 2), 0.5, 24, 20)])
+@pytest.mark.parametrize("proj,bricks,step,W,H", [(wl.PROJ_ORTHO, (1, 1, 1), 1.0, 30, 24), (wl.PROJ_PERSP, (2, 2, 2), 1.0, 28, 22),
+                                                  (wl.PROJ_ORTHO, (3, 1, 2), 0.5, 22, 18)])
 def test_measure_sector_count_equals_numpy_enumeration(vr, oracle, proj, bricks, step, W, H):
     """The roofline numerator's instrument (vr_measure's sector bitmap, 32 B x distinct sectors) pinned against an
     independent enumeration: numpy lists the footprints of the oracle's sample positions, maps them through the
@@ -333,15 +334,17 @@ def test_measure_sector_count_equals_numpy_enumeration(vr, oracle, proj, bricks,
     vol = vr.Volume(cube)
     vol.vr_set_transfer_function(wl.tf_ramp(0.15), -3.0, 8.0)
     vol.vr_set_bricks(*bricks)
-    samples, units = vol.vr_measure_units(vr.camera_from_spec(cs), W, H, step, 0, 0.0)
+    (samples, evaluated), units = vol.vr_measure_units(vr.camera_from_spec(cs), W, H, step, 0, 0.0)
     s2, sectors = vol.vr_measure(vr.camera_from_spec(cs), W, H, step, 0, 0.0)
-    s3, units_mip = vol.vr_measure_units(vr.camera_from_spec(cs), W, H, step, 1, 0.0)
+    (s3, e3), units_mip = vol.vr_measure_units(vr.camera_from_spec(cs), W, H, step, 1, 0.0)
     vol.close()
+    assert evaluated == samples and e3 == s3 and units[3] == 0     # tf_ramp has alpha > 0 from entry 1: no skipping
+    units, units_mip = units[:3], units_mip[:3]
     must, may, _ = _footprint_units(oracle, dims, cs, W, H, step, eps=2e-4)
-    total = ((70 + 8) // 8) * ((45 + 8) // 8) * ((52 + 8) // 8) * 64
+    total = ((70 + 9) // 8) * ((45 + 9) // 8) * ((52 + 9) // 8) * 64
     print(f"sectors gpu {units} numpy must {must} may {may} of {total}")
     assert sectors == units[0] and s2 == samples == s3 and units_mip == units
-    assert must[0] < 0.9 * total                           # sparse enough to be a test
+    assert must[0] < 0.92 * total                          # sparse enough to be a test
     for k in range(3):
         assert must[k] <= units[k] <= may[k], (k, must, units, may)
         assert may[k] - must[k] <= max(2, 0.002 * must[k])  # the bracket is tight: equality up to a few ties
@@ -404,4 +407,76 @@ def test_subcube_and_channel_range_match_oracle(vr, oracle):
         vol.vr_set_subcube((0, 0, 0), (71, 45, 52))
     with pytest.raises(vr.VrError):
         vol.vr_set_subcube((5, 0, 0), (4, 45, 52))
+    vol.close()
+
+
+# ---------------------------------------------------------------- NEXT-2 empty-space skipping ------------
+@pytest.mark.parametrize("cfg", [2, 3, 5])
+def test_empty_space_skipping_leaves_the_frame_bit_identical(vr, oracle, cfg):
+    """NEXT-2: cells whose samples contribute exactly nothing under the current table are
+    passed over.  The frame must be BIT-IDENTICAL with skipping on and off (only exact zeros are dropped), the
+    oracle gate holds unchanged, the lattice count is the oracle's, and fewer samples are evaluated."""
+    import torch
+    w = wl.config(cfg).scaled(1.0 / 8, W=192, H=160)
+    cube = w.cube("cuda")
+    cube[5:9, 10:20, 30:50] = float("nan")                       # a blanked block: its cells are empty as well
+    host = cube.cpu().numpy()
+    vol = vr.Volume(cube)
+    vol.vr_set_transfer_function(w.table, w.vmin, w.vmax)
+    info = vol.vr_get_skip_info()
+    assert info["active"] and 0.0 < info["occupied_fraction"] < 0.9 and info["mask_bytes"] > 0, info
+    for bricks, proj, step, ert in (((1, 1, 1), wl.PROJ_ORTHO, 1.0, 0.0), ((2, 2, 2), wl.PROJ_PERSP, 0.5, 0.0),
+                                    ((3, 1, 2), wl.PROJ_PERSP, 1.0, 0.995), ((2, 2, 2), wl.PROJ_ORTHO, 0.25, 0.9)):
+        vol.vr_set_bricks(*bricks)
+        cs = wl.orbit_camera(w.dims, 130.0, 20.0, proj)
+        cam = vr.camera_from_spec(cs)
+        vol.vr_set_empty_space_skipping(True)
+        on = vol.vr_render(cam, w.W, w.H, step, 0, ert).clone()
+        (vis_on, ev_on), u_on = vol.vr_measure_units(cam, w.W, w.H, step, 0, ert)
+        vol.vr_set_empty_space_skipping(False)
+        off = vol.vr_render(cam, w.W, w.H, step, 0, ert).clone()
+        (vis_off, ev_off), u_off = vol.vr_measure_units(cam, w.W, w.H, step, 0, ert)
+        torch.cuda.synchronize()
+        assert torch.equal(on.view(torch.int32), off.view(torch.int32)), (cfg, bricks, (on - off).abs().max().item())
+        ref = oracle.render(host, w.table, w.vmin, w.vmax, bricks, ocam(oracle, cs), w.W, w.H, step, 0, ert, route=1)
+        gate = TOL_ERT if ert > 0 else TOL_EA
+        assert np.abs(on.cpu().numpy() - ref["rgba"]).max() <= gate
+        assert vis_on == vis_off == ev_off == ref["samples"]       # the lattice walk and the termination point are unchanged
+        assert ev_on < 0.9 * vis_on and u_on[0] < u_off[0] and u_on[3] > 0 and u_off[3] == 0
+        print(f"cfg {cfg} bricks {bricks} step {step}: evaluated {ev_on / vis_on:.3f} of the lattice samples, "
+              f"cube sectors {u_on[0] / u_off[0]:.3f} of the unskipped frame")
+    vol.close()
+
+
+def test_mask_follows_the_transfer_function(vr, oracle):
+    """The mask is keyed to the table: after a table change the next frame equals a fresh volume's frame (bit for
+    bit) and the oracle's; tables without a transparent leading run and MIP frames do not use the mask."""
+    import torch
+    dims = (70, 45, 52)
+    cube = wl.cube_blobs(dims, 31, "cuda", n_blobs=6, amp=6.0, sigma=5.0)
+    host = cube.cpu().numpy()
+    cs = wl.orbit_camera(dims, 40.0, 25.0, wl.PROJ_PERSP)
+    cam = vr.camera_from_spec(cs)
+    W, H = 120, 90
+    t_lo = wl.tf_piecewise(-3.0, 8.0, [(0.5, 0.0), (3.0, 0.3)])
+    t_hi = wl.tf_piecewise(-3.0, 8.0, [(2.5, 0.0), (6.0, 0.5)])
+    vol = vr.Volume(cube)
+    frames, fracs = {}, {}
+    for name, tab, rng in (("lo", t_lo, (-3.0, 8.0)), ("hi", t_hi, (-3.0, 8.0)), ("hi_range", t_hi, (-2.0, 9.0)),
+                           ("lo_again", t_lo, (-3.0, 8.0))):
+        vol.vr_set_transfer_function(tab, *rng)
+        frames[name] = vol.vr_render(cam, W, H, 0.5, 0, 0.0).clone()
+        fracs[name] = vol.vr_get_skip_info()["occupied_fraction"]
+        fresh = vr.Volume(cube)
+        fresh.vr_set_transfer_function(tab, *rng)
+        f2 = fresh.vr_render(cam, W, H, 0.5, 0, 0.0)
+        torch.cuda.synchronize()
+        assert torch.equal(frames[name], f2), name
+        fresh.close()
+        ref = oracle.render(host, tab, rng[0], rng[1], (1, 1, 1), ocam(oracle, cs), W, H, 0.5, 0, 0.0)["rgba"]
+        assert np.abs(frames[name].cpu().numpy() - ref).max() <= TOL_EA, name
+    assert fracs["hi"] < fracs["lo"] and fracs["lo_again"] == fracs["lo"] and fracs["hi_range"] != fracs["hi"]
+    assert torch.equal(frames["lo"], frames["lo_again"])
+    vol.vr_set_transfer_function(wl.tf_ramp(0.2), -3.0, 8.0)      # alpha > 0 from entry 1 on: nothing is provably empty
+    assert not vol.vr_get_skip_info()["active"]
     vol.close()
