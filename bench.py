@@ -38,8 +38,9 @@ UNIT = "ms/frame"
 # Per-launch DRAM traffic of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum of one
 # `ncu --set full` capture), keyed by the run it was captured on; any other run reports traffic = null.
 NCU_TRAFFIC = {
-    # (config, image, mode, bricks): (bytes per launch, profiles/ file the number comes from)
-    (3, 1024, 0, (2, 2, 2)): (27.19e9, "profiles/r01cd_cast_full.md (r01d, mean of launches az 10 / 20 deg)"),
+    # (config, image, mode, bricks, skipping): (bytes per launch, profiles/ file the number comes from)
+    (3, 1024, 0, (2, 2, 2), True): (21.07e9, "profiles/r02_cast_full.md (r02d, mean of launches az 10 / 20 deg)"),
+    (3, 1024, 0, (2, 2, 2), False): (27.19e9, "profiles/r01cd_cast_full.md (r01d, mean of launches az 10 / 20 deg)"),
 }
 
 
@@ -160,6 +161,8 @@ def run_ours(args):
     relayout_ms, tiled_bytes = vol.vr_volume_info()
     vol.vr_set_transfer_function(w.table, w.vmin, w.vmax)
     vol.vr_set_bricks(*w.bricks)
+    vol.vr_set_empty_space_skipping(not args.no_skip)
+    skip_info = vol.vr_get_skip_info()                           # builds the occupancy mask once (a per-table step)
     B = w.bricks[0] * w.bricks[1] * w.bricks[2]
     cams = [vr.camera_from_spec(w.camera(az_deg=a)) for a in views]
     out = torch.empty((w.H, w.W, 4), dtype=torch.float32, device="cuda")
@@ -227,17 +230,31 @@ def run_ours(args):
             dist.destroy_process_group()
         return
 
-    # ---- untimed instrumented pass: samples evaluated and distinct 32-byte sectors per view ----
+    # ---- untimed instrumented pass: samples and distinct 32-byte sectors (cube + occupancy mask) per view ----
     used_views = sorted(set(view_of(k) for k in range(K)))
-    meas = {}
-    for v in used_views:
-        meas[v] = vol.vr_measure(cams[v], w.W, w.H, w.step, w.mode, w.ert_alpha)
-    samples = sum(meas[view_of(k)][0] for k in range(K))
-    alg_bytes = 32.0 * sum(meas[view_of(k)][1] for k in range(K))
+    meas = {v: vol.vr_measure_units(cams[v], w.W, w.H, w.step, w.mode, w.ert_alpha) for v in used_views}
+    samples = sum(meas[view_of(k)][0][0] for k in range(K))           # lattice samples visited (the oracle's count)
+    evaluated = sum(meas[view_of(k)][0][1] for k in range(K))         # of which not passed over by empty-space skipping
+    alg_bytes = 32.0 * sum(meas[view_of(k)][1][0] + meas[view_of(k)][1][3] for k in range(K))
     cast_total_ms = float(sum(cast_ms))
     peak, peak_src = measured_peak_gbs()
     achieved = alg_bytes / (cast_total_ms * 1e-3) / 1e9
     ms_per_frame = replicas.aggregate_ms_per_frame(total_ms, K, world)   # whole job: all ranks' frames
+
+    # ---- the same frames with skipping off (dense walk), untimed for the headline: what skipping buys ----
+    dense = None
+    if skip_info["active"]:
+        vol.vr_set_empty_space_skipping(False)
+        d_cast = []
+        for k in range(K):
+            vol.vr_render(cams[view_of(k)], w.W, w.H, w.step, w.mode, w.ert_alpha, out=out)
+            d_cast.append(vol.vr_get_stage_ms()[0])
+        d_meas = {v: vol.vr_measure_units(cams[v], w.W, w.H, w.step, w.mode, w.ert_alpha) for v in used_views}
+        d_bytes = 32.0 * sum(d_meas[view_of(k)][1][0] for k in range(K))
+        vol.vr_set_empty_space_skipping(True)
+        d_ach = d_bytes / (sum(d_cast) * 1e-3) / 1e9
+        dense = {"cast_ms": float(sum(d_cast)) / K, "algorithmic_bytes_per_launch": d_bytes / K, "achieved": d_ach,
+                 "frac": d_ach / peak, "note": "vr_set_empty_space_skipping(0): every lattice sample is evaluated; same frames bit for bit"}
 
     # ---- the oracle beside it: one full frame (view az 30 deg) on the host cores ----
     cpu = None
@@ -268,7 +285,8 @@ def run_ours(args):
                   "gate": 5e-3 if w.ert_alpha > 0 else 1e-4}
         del host_cube
 
-    traffic, traffic_src = NCU_TRAFFIC.get((args.config, w.W if w.W == w.H else -1, w.mode, tuple(w.bricks)), (None, None))
+    traffic, traffic_src = NCU_TRAFFIC.get((args.config, w.W if w.W == w.H else -1, w.mode, tuple(w.bricks),
+                                            bool(skip_info["active"])), (None, None))
     cfg = describe(w, views)
     cfg["views_timed"] = {"count": len(used_views), "azimuths_deg": [views[v] for v in used_views],
                           "note": "view k of the timed region is azimuth views[k mod len(views)]; steps < len(views) time a prefix of the orbit"}
@@ -280,7 +298,9 @@ def run_ours(args):
         "ms_per_frame_min": min(per_frame), "ms_per_frame_max": max(per_frame),
         "ms_per_view": {str(int(views[view_of(k)])): round(per_frame[k], 3) for k in range(K)},
         "gsamples_per_s": samples / (total_ms * 1e-3) / 1e9 * world,
-        "samples_per_frame": samples / K,
+        "samples_per_frame": samples / K, "samples_evaluated_per_frame": evaluated / K,
+        "gsamples_evaluated_per_s": evaluated / (total_ms * 1e-3) / 1e9 * world,
+        "empty_space_skipping": dict(skip_info, dense=dense),
         "stages_ms": {"cast": cast_total_ms / K, "composite": float(sum(comp_ms)) / K},
         "relayout": {"ms": relayout_ms, "GBps_read_plus_write": (4.0 * cube.numel() + tiled_bytes) / (relayout_ms * 1e-3) / 1e9
                      if relayout_ms > 0 else None},
@@ -288,14 +308,14 @@ def run_ours(args):
         "e2e": {"value": replicas.aggregate_ms_per_frame(e2e_ms, K, world), "unit": UNIT, "h2d_bytes_per_step": B * (72 + 4) + 256,
                 "d2h_bytes_per_step": w.W * w.H * 16,
                 "note": "vr_render_to_host: per-frame plan upload + kernels + D2H of the RGBA frame into pinned host memory"},
-        "gpu_launches": 2 * K if B > 1 or w.mode == 1 else K,
+        "gpu_launches": 2 * K if B > 1 or w.mode == 1 else K,          # cast_kernel (+ composite_kernel) per frame
         "roofline": {"bound": "hbm", "kernel": "cast_kernel<EA>" if w.mode == 0 else "cast_kernel<MIP>",
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": alg_bytes / K,
                      "cube_bytes": 4.0 * cube.numel(), "avg_launch_ms": cast_total_ms / K,
-                     "definition": "32 B x distinct sectors of the tiled cube touched by the frame's samples "
-                                   "(instrumented pass, untimed) / cast kernel time (CUDA events)"},
+                     "definition": "32 B x distinct sectors of the tiled cube and of the occupancy mask touched by the "
+                                   "frame's evaluated samples (instrumented pass, untimed) / cast kernel time (CUDA events)"},
         "cpu_baseline": cpu, "parity": parity,
         "paper_context": "< 0.3 s per 1024^2 frame of the 26 GB GASS cube on 3 workstations / 8 Tesla C1060 "
                          "(PAPER.md:9,304): another machine and the real cube, context only",
@@ -364,6 +384,7 @@ def run_sweep(args):
     torch.cuda.synchronize()
     vol = vr.Volume(cube)
     vol.vr_set_transfer_function(w.table, w.vmin, w.vmax)
+    vol.vr_set_empty_space_skipping(not args.no_skip)
     cs = wl.orbit_camera(w.dims, 30.0, 20.0, wl.PROJ_ORTHO)
     cam = vr.camera_from_spec(cs)
     peak, peak_src = measured_peak_gbs()
@@ -389,7 +410,8 @@ def run_sweep(args):
             cast.append(vol.vr_get_stage_ms()[0])
         torch.cuda.synchronize()
         ms = sorted(ev[2 * k].elapsed_time(ev[2 * k + 1]) for k in range(reps))
-        samples, sectors = vol.vr_measure(cam, size, size, step, mode, 0.0)
+        (samples, evaluated), units = vol.vr_measure_units(cam, size, size, step, mode, 0.0)
+        sectors = units[0] + units[3]
         best, med = ms[0], ms[len(ms) // 2]
         cast_med = sorted(cast)[len(cast) // 2]
         B = bricks[0] * bricks[1] * bricks[2]
@@ -405,7 +427,7 @@ def run_sweep(args):
         print(json.dumps({"sweep_point": {"mode": "MIP" if mode else "EA", "bricks": B, "step_voxels": step,
                                           "image": f"{size}x{size}"},
                           "ms_per_frame_best": best, "ms_per_frame_median": med, "cast_ms_median": cast_med,
-                          "samples": samples, "gsamples_per_s": samples / (med * 1e-3) / 1e9,
+                          "samples": samples, "samples_evaluated": evaluated, "gsamples_per_s": samples / (med * 1e-3) / 1e9,
                           "algorithmic_GB": 32e-9 * sectors, "bytes_per_sample": 32.0 * sectors / samples,
                           "hbm_GBps_algorithmic": 32e-9 * sectors / (cast_med * 1e-3),
                           "frac_of_peak": 32e-9 * sectors / (cast_med * 1e-3) / peak, "peak": peak,
@@ -426,6 +448,7 @@ def main():
                     help="oracle legs render every n-th pixel in x and y (default 1 = the full frame for cpu_baseline, 4 for --impl reference)")
     ap.add_argument("--image", type=int, default=None, help="override the image size (W = H), e.g. 512 for Fig 12's comparison")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-skip", action="store_true", help="vr_set_empty_space_skipping(0): the dense walk (same frames)")
     ap.add_argument("--l2-fetch", type=int, default=None, choices=[32, 64, 128],
                     help="device-wide L2 fetch granularity hint in bytes (vr_set_l2_fetch_granularity); default: leave as is")
     ap.add_argument("--sweep", action="store_true", help="run BASELINE.json configs[4] (28 points) instead of the headline")

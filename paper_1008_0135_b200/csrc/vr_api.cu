@@ -64,6 +64,7 @@ struct vr_volume {
     size_t frame_floats = 0;
 
     // NEXT-2 empty-space skipping: occupancy mask (one bit per voxel cell), built for the current table on demand
+    int seg_max = 64;                 // samples (and voxels of path) per anchored segment; env VR_SEG overrides (1..64)
     bool skip_enabled = true;
     unsigned long long* d_mask = nullptr;
     unsigned long long* d_mask_count = nullptr;
@@ -135,7 +136,7 @@ vr_status build_frame(const vr_volume* vol, const vr_camera* cam, int W, int H, 
     P.ert_on = (ert > 0.0f && ert < 1.0f) ? 1 : 0;
     P.ert = ert;
     // segments of <= 64 voxels of path (sampler.cuh): fp32 positions stay within ~65 of their anchor
-    P.seg_len = std::max(1, std::min(64, (int)(64.0 / (double)step)));
+    P.seg_len = std::max(1, std::min(vol->seg_max, (int)((double)vol->seg_max / (double)step)));
     P.seg_span = (int)std::ceil((double)P.seg_len * (double)step) + 1;
     P.nbx = vol->NBX; P.nby = vol->NBY;
     P.x_zero_below = table_zero_below(vol);   // the per-step opacity correction keeps zeros zero
@@ -296,6 +297,10 @@ vr_status vr_create_volume(const int dims[3], const float* d_data, vr_volume** o
     vr_volume* v = new (std::nothrow) vr_volume();
     if (!v) return fail(VR_ERR_OOM, "vr_create_volume: host allocation failed");
     for (int a = 0; a < 3; ++a) { v->dims[a] = dims[a]; v->sub_hi[a] = dims[a]; }
+    if (const char* e_ = std::getenv("VR_SEG")) {          // tuning knob for measurements
+        const int sv = std::atoi(e_);
+        if (sv >= 1 && sv <= 64) v->seg_max = sv;
+    }
     v->TX = (dims[0] + 2 + 7) / 8; v->TY = (dims[1] + 2 + 7) / 8; v->TZ = (dims[2] + 2 + 7) / 8;   // padded: +1 layer each side
     if ((double)v->TX * v->TY * vr::TILE_ELEMS >= 1073741824.0) {   // slab bytes and in-slab offsets stay 32-bit
         delete v;
