@@ -224,16 +224,20 @@ typedef struct {
     double M;    /* MIP: running maximum, -inf initially */
 } accum;
 
-/* samples i_lo <= i < i_hi of the global lattice t_i = t_near + (i + 1/2) step (O4) */
-static long long march(const float* data, const int dims[3], const double tab[256][4], double vmin,
-                       double vmax, const double o[3], const double d[3], double t_near,
-                       double step, long long i_lo, long long i_hi, int mode, double ert,
-                       accum* acc) {
-    long long count = 0;
-    int ert_on = (ert > 0.0 && ert < 1.0);
+static void accum_reset(accum* acc) {
     acc->C[0] = acc->C[1] = acc->C[2] = 0.0;
     acc->A = 0.0;
     acc->M = -INFINITY;
+}
+
+/* samples i_lo <= i < i_hi of the global lattice t_i = t_near + (i + 1/2) step (O4), continuing the accumulation
+ * in *acc; returns the number of samples taken and sets *terminated when O7 stopped the ray */
+static long long march(const float* data, const int dims[3], const double tab[256][4], double vmin,
+                       double vmax, const double o[3], const double d[3], double t_near,
+                       double step, long long i_lo, long long i_hi, int mode, double ert,
+                       accum* acc, int* terminated) {
+    long long count = 0;
+    int ert_on = (ert > 0.0 && ert < 1.0);
     for (long long i = i_lo; i < i_hi; ++i) {
         double t = t_near + ((double)i + 0.5) * step;
         double p[3] = {o[0] + t * d[0], o[1] + t * d[1], o[2] + t * d[2]};
@@ -250,9 +254,46 @@ static long long march(const float* data, const int dims[3], const double tab[25
             acc->C[1] += wgt * e[1];
             acc->C[2] += wgt * e[2];
             acc->A += wgt;
-            if (ert_on && acc->A >= ert) break;
+            if (ert_on && acc->A >= ert) { *terminated = 1; break; }
         }
     }
+    return count;
+}
+
+/* S2 channel mask ("enabling/disabling spectral channel(s)"): the enabled channels form maximal runs
+ * [za, zb) of consecutive channels; a lattice sample is taken iff it is owned, by O9's rule, by the slab
+ * [za, zb] of some run (intersected with the box it is rendered in).  One run [0, nz) = no mask. */
+typedef struct { int za, zb; } zrun;
+typedef struct { double t_in; long long lo, hi; } span;
+static int cmp_span(const void* x, const void* y) {
+    const span* a = (const span*)x;
+    const span* b = (const span*)y;
+    return (a->lo > b->lo) - (a->lo < b->lo);
+}
+
+/* All samples of the lattice inside box [lo,hi] AND an enabled run, front to back, accumulated into *acc (reset
+ * here).  Returns samples taken; *t_first = entry parameter of the first non-empty span (sort key of O10);
+ * *any = 1 if at least one sample range was non-empty. */
+static long long march_box(const float* data, const int dims[3], const double tab[256][4], double vmin, double vmax,
+                           const double o[3], const double d[3], double t_near, double t_far, double step,
+                           const double lo[3], const double hi[3], const zrun* runs, int n_runs, span* work,
+                           int mode, double ert, accum* acc, double* t_first, int* any) {
+    int ns = 0;
+    for (int r = 0; r < n_runs; ++r) {
+        double blo[3] = {lo[0], lo[1], lo[2]}, bhi[3] = {hi[0], hi[1], hi[2]};
+        if (blo[2] < (double)runs[r].za) blo[2] = (double)runs[r].za;
+        if (bhi[2] > (double)runs[r].zb) bhi[2] = (double)runs[r].zb;
+        if (box_span(o, d, blo, bhi, step, t_near, t_far, &work[ns].t_in, &work[ns].lo, &work[ns].hi)) ++ns;
+    }
+    qsort(work, (size_t)ns, sizeof(span), cmp_span);
+    accum_reset(acc);
+    *any = ns > 0;
+    *t_first = ns > 0 ? work[0].t_in : 0.0;
+    long long count = 0;
+    int terminated = 0;
+    for (int k = 0; k < ns && !terminated; ++k)
+        count += march(data, dims, tab, vmin, vmax, o, d, t_near, step, work[k].lo, work[k].hi, mode, ert, acc,
+                       &terminated);
     return count;
 }
 
@@ -266,11 +307,11 @@ static int cmp_key(const void* x, const void* y) {
 }
 
 /* ---------------------------------------------------------------- O1-O11 pixels ----------- */
-int vro_render_pixels_sub(const float* data, const int dims[3], const float rgba[1024], float vmin_f,
-                          float vmax_f, const int bricks_in[3], const int sub_lo[3], const int sub_hi[3],
-                          const vro_camera* cam, int W, int H, float step_f, int mode, float ert_f, int route,
-                          long long n_pix, const int* px, const int* py, float* out_rgba, float* out_scalar,
-                          float* out_brick, long long* out_samples, int threads) {
+int vro_render_pixels_mask(const float* data, const int dims[3], const float rgba[1024], float vmin_f,
+                           float vmax_f, const int bricks_in[3], const int sub_lo[3], const int sub_hi[3],
+                           const unsigned char* chan_mask, const vro_camera* cam, int W, int H, float step_f, int mode,
+                           float ert_f, int route, long long n_pix, const int* px, const int* py, float* out_rgba,
+                           float* out_scalar, float* out_brick, long long* out_samples, int threads) {
     if (!data || !dims || !rgba || !cam || !out_rgba || n_pix < 0) return -1;
     /* S1 sub-cube ("a manual sub-cube", PAPER.md:138 channel enable/disable): only samples of the
      * global lattice that lie in [sub_lo, sub_hi) are taken; the lattice itself (O4) and the sampling (O5, whole
@@ -300,6 +341,23 @@ int vro_render_pixels_sub(const float* data, const int dims[3], const float rgba
     corrected_table(rgba, step, tstep);
     corrected_table(rgba, 1.0, traw);
 
+    /* S2: maximal runs of enabled channels (no mask: the single run [0, nz)) */
+    zrun* runs = malloc(sizeof(zrun) * (size_t)(dims[2] / 2 + 2));
+    if (!runs) { free(tabs); return -1; }
+    int n_runs = 0;
+    if (!chan_mask) {
+        runs[0].za = 0; runs[0].zb = dims[2]; n_runs = 1;
+    } else {
+        for (int z = 0; z < dims[2];) {
+            if (!chan_mask[z]) { ++z; continue; }
+            int z1 = z;
+            while (z1 < dims[2] && chan_mask[z1]) ++z1;
+            runs[n_runs].za = z; runs[n_runs].zb = z1; ++n_runs;
+            z = z1;
+        }
+    }
+    const int plain = (!chan_mask && !has_sub);   /* route 0 then marches [0, n) directly, as O4 states it */
+
     long long total = 0;
 #ifdef _OPENMP
     if (threads <= 0) threads = omp_get_max_threads();
@@ -313,17 +371,20 @@ int vro_render_pixels_sub(const float* data, const int dims[3], const float rgba
         long long n = vro_ray_extent(o, d, dims, step, &t_near, &t_far);
         accum fin;
         fin.C[0] = fin.C[1] = fin.C[2] = 0.0; fin.A = 0.0; fin.M = -INFINITY;
+        span work[n_runs > 0 ? n_runs : 1];
         if (route == 0) {
-            long long a_lo = 0, a_hi = n;
-            if (has_sub && n > 0) {
+            if (plain) {
+                int terminated = 0;
+                if (n > 0)
+                    total += march(data, dims, (const double(*)[4])tstep, vmin, vmax, o, d, t_near, step, 0, n, mode,
+                                   ert, &fin, &terminated);
+            } else if (n > 0) {                                /* S1 / S2: the sub-cube and the enabled runs */
                 double blo[3] = {(double)slo[0], (double)slo[1], (double)slo[2]};
                 double bhi[3] = {(double)shi[0], (double)shi[1], (double)shi[2]};
-                double t_in_unused;
-                if (!box_span(o, d, blo, bhi, step, t_near, t_far, &t_in_unused, &a_lo, &a_hi)) a_hi = a_lo = 0;
+                double t_first; int any;
+                total += march_box(data, dims, (const double(*)[4])tstep, vmin, vmax, o, d, t_near, t_far, step, blo,
+                                   bhi, runs, n_runs, work, mode, ert, &fin, &t_first, &any);
             }
-            if (a_hi > a_lo)
-                total += march(data, dims, (const double(*)[4])tstep, vmin, vmax, o, d, t_near,
-                               step, a_lo, a_hi, mode, ert, &fin);
         } else {
             brick_key keys[B > 0 ? B : 1];
             accum parts[B > 0 ? B : 1];
@@ -333,9 +394,7 @@ int vro_render_pixels_sub(const float* data, const int dims[3], const float rgba
                     for (int bi = 0; bi < bricks[0]; ++bi) {
                         int b = (bk * bricks[1] + bj) * bricks[0] + bi;
                         accum* part = &parts[b];
-                        part->C[0] = part->C[1] = part->C[2] = 0.0;
-                        part->A = 0.0; part->M = -INFINITY;
-                        double t_in; long long i_lo, i_hi;
+                        accum_reset(part);
                         int idx3[3] = {bi, bj, bk};
                         double blo[3], bhi[3];
                         brick_box(dims, bricks, idx3, blo, bhi);
@@ -343,10 +402,11 @@ int vro_render_pixels_sub(const float* data, const int dims[3], const float rgba
                             if (blo[a] < (double)slo[a]) blo[a] = (double)slo[a];
                             if (bhi[a] > (double)shi[a]) bhi[a] = (double)shi[a];
                         }
-                        if (n > 0 && box_span(o, d, blo, bhi, step, t_near, t_far, &t_in, &i_lo, &i_hi)) {
-                            total += march(data, dims, (const double(*)[4])tstep, vmin, vmax, o,
-                                           d, t_near, step, i_lo, i_hi, mode, ert, part);
-                            keys[nk].t_in = t_in; keys[nk].b = b; ++nk;
+                        if (n > 0) {
+                            double t_first; int any;
+                            total += march_box(data, dims, (const double(*)[4])tstep, vmin, vmax, o, d, t_near, t_far,
+                                               step, blo, bhi, runs, n_runs, work, mode, ert, part, &t_first, &any);
+                            if (any) { keys[nk].t_in = t_first; keys[nk].b = b; ++nk; }
                         }
                         if (out_brick) {
                             if (mode == VRO_MODE_MIP) {
@@ -391,8 +451,19 @@ int vro_render_pixels_sub(const float* data, const int dims[3], const float rgba
         }
     }
     free(tabs);
+    free(runs);
     if (out_samples) *out_samples = total;
     return 0;
+}
+
+int vro_render_pixels_sub(const float* data, const int dims[3], const float rgba[1024], float vmin,
+                          float vmax, const int bricks[3], const int sub_lo[3], const int sub_hi[3],
+                          const vro_camera* cam, int W, int H, float step, int mode, float ert_alpha, int route,
+                          long long n_pix, const int* px, const int* py, float* out_rgba, float* out_scalar,
+                          float* out_brick, long long* out_samples, int threads) {
+    return vro_render_pixels_mask(data, dims, rgba, vmin, vmax, bricks, sub_lo, sub_hi, NULL, cam, W, H, step, mode,
+                                  ert_alpha, route, n_pix, px, py, out_rgba, out_scalar, out_brick, out_samples,
+                                  threads);
 }
 
 int vro_render_pixels(const float* data, const int dims[3], const float rgba[1024], float vmin,

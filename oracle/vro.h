@@ -85,6 +85,18 @@ int vro_render_pixels_sub(const float* data, const int dims[3], const float rgba
                           long long n_pix, const int* px, const int* py, float* out_rgba, float* out_scalar,
                           float* out_brick, long long* out_samples, int threads);
 
+/* S2  Same with a spectral-channel mask ("enabling/disabling spectral channel(s)"): chan_mask[z] != 0
+ *     enables channel z (NULL = all enabled).  The enabled channels form maximal runs [za, zb); a lattice sample is
+ *     taken iff O9's ownership rule gives it to the slab [za, zb] of some run (intersected with the sub-cube and,
+ *     in route 1, the brick): each run is one more box, so a mask with a single run equals the sub-cube
+ *     {0,0,za}..{nx,ny,zb} of S1.  Lattice (O4) and sampling (O5, whole cube, all channels) are unchanged;
+ *     accumulation runs front to back through the runs' sample ranges, termination (O7) as before.            */
+int vro_render_pixels_mask(const float* data, const int dims[3], const float rgba[1024], float vmin,
+                           float vmax, const int bricks[3], const int sub_lo[3], const int sub_hi[3],
+                           const unsigned char* chan_mask, const vro_camera* cam, int W, int H, float step, int mode,
+                           float ert_alpha, int route, long long n_pix, const int* px, const int* py, float* out_rgba,
+                           float* out_scalar, float* out_brick, long long* out_samples, int threads);
+
 /* Full frame: every pixel, row-major [py][px].  out_brick then is [B][H][W][4] / [B][H][W].      */
 int vro_render(const float* data, const int dims[3], const float rgba[1024], float vmin,
                float vmax, const int bricks[3], const vro_camera* cam, int W, int H, float step,

@@ -55,6 +55,11 @@ def lib():
                                                C.c_longlong, i3, i3, fp, fp, fp,
                                                C.POINTER(C.c_longlong), C.c_int]
         _lib.vro_render_pixels_sub.restype = C.c_int
+        _lib.vro_render_pixels_mask.argtypes = [fp, i3, fp, C.c_float, C.c_float, i3, i3, i3, C.POINTER(C.c_ubyte),
+                                                C.POINTER(Camera), C.c_int, C.c_int, C.c_float, C.c_int, C.c_float,
+                                                C.c_int, C.c_longlong, i3, i3, fp, fp, fp,
+                                                C.POINTER(C.c_longlong), C.c_int]
+        _lib.vro_render_pixels_mask.restype = C.c_int
         _lib.vro_max_threads.argtypes = []
         _lib.vro_max_threads.restype = C.c_int
     return _lib
@@ -137,8 +142,9 @@ def brick_span(o, d, dims, bricks, ijk, step, t_near, t_far):
 
 
 def render_pixels(data, rgba, vmin, vmax, bricks, cam, W, H, step, mode, ert_alpha, route, px, py,
-                  want_bricks=False, threads=0, subcube=None):
-    """Render the listed pixels.  Returns dict(rgba [n,4], scalar [n] (MIP), bricks, samples)."""
+                  want_bricks=False, threads=0, subcube=None, chan_mask=None):
+    """Render the listed pixels.  Returns dict(rgba [n,4], scalar [n] (MIP), bricks, samples).
+    chan_mask: None or nz values, non-zero = channel enabled (rule S2)."""
     a, dims = _cube(data)
     t = np.ascontiguousarray(rgba, dtype=np.float32).reshape(1024)
     px = np.ascontiguousarray(px, dtype=np.int32).reshape(-1)
@@ -156,8 +162,13 @@ def render_pixels(data, rgba, vmin, vmax, bricks, cam, W, H, step, mode, ert_alp
     ip = C.POINTER(C.c_int)
     sub_lo = _i3(subcube[0]) if subcube is not None else None
     sub_hi = _i3(subcube[1]) if subcube is not None else None
-    rc = lib().vro_render_pixels_sub(
-        _fp(a), _i3(dims), _fp(t), float(vmin), float(vmax), _i3(bricks), sub_lo, sub_hi, C.byref(cam), int(W),
+    cm = None
+    if chan_mask is not None:
+        cm_arr = np.ascontiguousarray(np.asarray(chan_mask) != 0, dtype=np.uint8)
+        assert cm_arr.size == dims[2]
+        cm = cm_arr.ctypes.data_as(C.POINTER(C.c_ubyte))
+    rc = lib().vro_render_pixels_mask(
+        _fp(a), _i3(dims), _fp(t), float(vmin), float(vmax), _i3(bricks), sub_lo, sub_hi, cm, C.byref(cam), int(W),
         int(H), float(step), int(mode), float(ert_alpha), int(route), n,
         px.ctypes.data_as(ip), py.ctypes.data_as(ip), _fp(out),
         _fp(scalar) if scalar is not None else None, _fp(ob) if ob is not None else None,
@@ -168,11 +179,11 @@ def render_pixels(data, rgba, vmin, vmax, bricks, cam, W, H, step, mode, ert_alp
 
 
 def render(data, rgba, vmin, vmax, bricks, cam, W, H, step, mode, ert_alpha=0.0, route=0,
-           want_bricks=False, threads=0, subcube=None):
+           want_bricks=False, threads=0, subcube=None, chan_mask=None):
     """Full frame; arrays come back shaped [H, W, ...] (py = 0 is the bottom row)."""
     yy, xx = np.meshgrid(np.arange(H, dtype=np.int32), np.arange(W, dtype=np.int32), indexing="ij")
     r = render_pixels(data, rgba, vmin, vmax, bricks, cam, W, H, step, mode, ert_alpha, route,
-                      xx.reshape(-1), yy.reshape(-1), want_bricks, threads, subcube)
+                      xx.reshape(-1), yy.reshape(-1), want_bricks, threads, subcube, chan_mask)
     r["rgba"] = r["rgba"].reshape(H, W, 4)
     if r["scalar"] is not None:
         r["scalar"] = r["scalar"].reshape(H, W)
