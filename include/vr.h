@@ -54,6 +54,7 @@ typedef struct {
 } vr_camera;
 
 #define VR_MAX_BRICKS 512 /* bx*by*bz */
+#define VR_MAX_CHANNEL_RUNS 16 /* runs of consecutive enabled channels a channel mask may have */
 
 /* a0  Brick partitioner / tiled re-layout ("loads its portion").
  *     Copies the linear cube d_data[nz][ny][nx] into the library's own tiled layout (8x8x8-voxel
@@ -85,6 +86,15 @@ vr_status vr_set_bricks(vr_volume* vol, int bx, int by, int bz);
  *     across the sub-cube's faces) are unchanged: the sub-cube is one more box every brick is intersected with
  *     (S1).  NULL, NULL restores the whole cube.  INVALID_ARG unless 0 <= lo_a <= hi_a <= n_a.       */
 vr_status vr_set_subcube(vr_volume* vol, const int lo[3], const int hi[3]);
+
+/* Spectral-channel mask ("enabling/disabling spectral channel(s)"): enabled[z] != 0 keeps channel z,
+ *     HOST array of nz bytes, copied; NULL enables every channel again.  The enabled channels form maximal runs
+ *     [za, zb) of consecutive channels, and a sample of the ray lattice is taken iff it lies in the slab
+ *     za <= z <= zb of some run — decided in double precision with the rule that assigns samples to bricks
+ *     (S2, O9), so a mask with one run equals vr_set_subcube on that z range.  The lattice and the
+ *     sampling (which reads neighbouring channels across a run's faces) are unchanged.  Combines with bricks, the
+ *     sub-cube, both modes and early termination.  INVALID_ARG: more than VR_MAX_CHANNEL_RUNS runs.             */
+vr_status vr_set_channel_mask(vr_volume* vol, const unsigned char* enabled);
 
 /* NEXT-2  Empty-space skipping keyed to the transfer function ("keeping the size of these tasks
  *     balanced"; PAPER.md:205 the work "varies based on the dataset characteristics"; PAPER.md:294 transfer functions

@@ -35,6 +35,7 @@ constexpr int CTA_W = VR_CTA_W;               // a CTA renders a CTA_W x CTA_H p
 constexpr int CTA_H = VR_CTA_H;
 constexpr int CTA_THREADS = CTA_W * CTA_H;
 constexpr int MODE_EA = 0, MODE_MIP = 1;
+constexpr int MAX_RUNS = 16;                  // VR_MAX_CHANNEL_RUNS of include/vr.h
 
 struct FrameParams {
     double eye[3], right[3], up[3], fwd[3];   // O1
@@ -50,6 +51,8 @@ struct FrameParams {
     int ert_on;
     int seg_len, seg_span;                    // samples per anchored segment; ceil(seg_len*step)+1 (sampler.cuh)
     int nbx, nby;                             // occupancy-mask words (4^3 cells) per row / per column
+    int n_runs;                               // S2 channel mask: runs of enabled channels (0 = no mask)
+    int run_z[2 * MAX_RUNS];                  // [za, zb) per run, ascending
 };
 
 struct BrickRec {
@@ -348,14 +351,50 @@ build_mask_kernel(const float* __restrict__ vol, unsigned ty_stride, unsigned sl
     }
 }
 
+// bits [lo, hi) of a 64-bit set kept as two words, 0 <= lo, hi <= 64
+__device__ __forceinline__ void range_bits(int lo, int hi, unsigned& b_lo, unsigned& b_hi) {
+    const unsigned long long m_hi = hi >= 64 ? ~0ull : ((1ull << hi) - 1ull);
+    const unsigned long long m_lo = lo >= 64 ? ~0ull : ((1ull << lo) - 1ull);
+    const unsigned long long m = hi > lo ? (m_hi & ~m_lo) : 0ull;
+    b_lo = (unsigned)m; b_hi = (unsigned)(m >> 32);
+}
+
+// S2 channel mask: samples jl in [0, je) of the segment starting at lattice index i_seg that are owned
+// (O9's rule, double precision, the oracle's expressions) by the slab [za, zb] of some run of enabled channels.
+// Only runs that can reach the segment's z-range cost the two divisions.
+__device__ __forceinline__ void channel_bits(const FrameParams& P, const double o[3], const double d[3], double t_near,
+                                             long long i_seg, int je, unsigned& b_lo, unsigned& b_hi) {
+    b_lo = b_hi = 0u;
+    const double z_a = o[2] + (t_near + ((double)i_seg + 0.5) * P.step) * d[2];
+    const double z_b = o[2] + (t_near + ((double)(i_seg + je - 1) + 0.5) * P.step) * d[2];
+    const double z_min = fmin(z_a, z_b) - 1.0, z_max = fmax(z_a, z_b) + 1.0;
+    for (int r = 0; r < P.n_runs; ++r) {
+        const double za = (double)P.run_z[2 * r], zb = (double)P.run_z[2 * r + 1];
+        if (zb < z_min || za > z_max) continue;
+        int lo = 0, hi = je;
+        if (d[2] == 0.0) {
+            if (!(za <= o[2] && o[2] < zb)) continue;                       // O3's rule for a ray parallel to the planes
+        } else {
+            const double t0 = (za - o[2]) / d[2], t1 = (zb - o[2]) / d[2];
+            const double ta = t0 < t1 ? t0 : t1, tb = t0 < t1 ? t1 : t0;
+            const long long ia = lattice_index(ta, t_near, P.step) - i_seg, ib = lattice_index(tb, t_near, P.step) - i_seg;
+            lo = (int)(ia < 0 ? 0 : (ia > je ? je : ia));
+            hi = (int)(ib < 0 ? 0 : (ib > je ? je : ib));
+        }
+        unsigned m_lo, m_hi;
+        range_bits(lo, hi, m_lo, m_hi);
+        b_lo |= m_lo; b_hi |= m_hi;
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // a1 + a3 + a4/a5  the caster.  grid.x = sum over bricks of the CTA_W x CTA_H pixel tiles (16x8) of their
 // rendering rectangles; block = 128 threads = 4 warps, each an 8x4-pixel patch.
-// SKIP = 1 consults the occupancy mask (EA only).  INSTR = 1 is the measuring build (samples, sector bitmaps),
+// SKIP = 1 consults the occupancy mask (EA only); CHAN = 1 applies the channel mask (S2).  INSTR = 1 is the measuring build (samples, sector bitmaps),
 // never the product path; it walks the same cells and takes the same skip and termination decisions.
 // counters (INSTR): [0] lattice samples visited (the oracle's count), [1] samples evaluated (not skipped).
 // ------------------------------------------------------------------------------------------------
-template <int MODE, int INSTR, int SKIP>
+template <int MODE, int INSTR, int SKIP, int CHAN>
 __global__ void __launch_bounds__(CTA_THREADS, VR_CAST_MINBLOCKS)
 cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ bricks, int n_bricks,
             const float* __restrict__ vol, const float4* __restrict__ tf_global, const unsigned long long* __restrict__ mask,
@@ -438,7 +477,10 @@ cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ 
             Anchor An;
             set_anchor(o, d, t_near, P.step, i_lo + js, h, P.seg_span, An);
             const int je = min(n - js, P.seg_len);
+            unsigned en_lo = 0xffffffffu, en_hi = 0xffffffffu;
+            if (CHAN) channel_bits(P, o, d, t_near, i_lo + js, je, en_lo, en_hi);
             for (int jl = 0; jl < je; ++jl) {
+                if (CHAN && !(((jl < 32 ? en_lo : en_hi) >> (jl & 31)) & 1u)) continue;   // S2: channel disabled
                 Cell c;
                 locate(An, jl, h, c);
                 ++visited;
@@ -476,13 +518,23 @@ cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ 
             Anchor An;
             set_anchor(o, d, t_near, P.step, i_lo + js, h, P.seg_span, An);
             const int je = min(n - js, P.seg_len);
-            if (SKIP) {
-                unsigned todo_lo = 0u, todo_hi = 0u;          // bit jl: sample jl of this segment can contribute
-                for (int jl = 0; jl < je; ++jl) {
-                    unsigned ix, iy, iz;
-                    locate_cell(An, jl, h, ix, iy, iz);
-                    const unsigned occ = cell_occupied(mask, nbx, nbxy, ix, iy, iz, mc) ? 1u : 0u;
-                    if (jl < 32) todo_lo |= occ << jl; else todo_hi |= occ << (jl - 32);
+            if (SKIP || CHAN) {
+                unsigned todo_lo, todo_hi;                     // bit jl: sample jl of this segment is to be evaluated
+                range_bits(0, je, todo_lo, todo_hi);
+                if (CHAN) {                                    // S2: channels the user disabled
+                    unsigned en_lo, en_hi;
+                    channel_bits(P, o, d, t_near, i_lo + js, je, en_lo, en_hi);
+                    todo_lo &= en_lo; todo_hi &= en_hi;
+                }
+                if (SKIP) {                                    // NEXT-2: cells that cannot contribute
+                    unsigned occ_lo = 0u, occ_hi = 0u;
+                    for (int jl = 0; jl < je; ++jl) {
+                        unsigned ix, iy, iz;
+                        locate_cell(An, jl, h, ix, iy, iz);
+                        const unsigned occ = cell_occupied(mask, nbx, nbxy, ix, iy, iz, mc) ? 1u : 0u;
+                        if (jl < 32) occ_lo |= occ << jl; else occ_hi |= occ << (jl - 32);
+                    }
+                    todo_lo &= occ_lo; todo_hi &= occ_hi;
                 }
                 while (todo_lo | todo_hi) {
                     int jl;
@@ -492,8 +544,12 @@ cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ 
                     locate(An, jl, h, c);
                     const float v = sample_cached(vol_base, P.ty_stride, slab_bytes, c, K);
                     if (have) {
-                        classify_blend(tf, P, vprev, Cr, Cg, Cb, A);
-                        if (P.ert_on && A >= P.ert) { done = true; break; }
+                        if (MODE == MODE_EA) {
+                            classify_blend(tf, P, vprev, Cr, Cg, Cb, A);
+                            if (P.ert_on && A >= P.ert) { done = true; break; }
+                        } else {
+                            M = fmaxf(M, vprev);
+                        }
                     }
                     vprev = v; have = true;
                 }

@@ -64,6 +64,8 @@ struct vr_volume {
     size_t frame_floats = 0;
 
     // NEXT-2 empty-space skipping: occupancy mask (one bit per voxel cell), built for the current table on demand
+    int n_runs = 0;                   // S2 channel mask as runs of enabled channels; 0 = every channel enabled
+    int run_z[2 * vr::MAX_RUNS] = {0};
     int seg_max = 64;                 // samples (and voxels of path) per anchored segment; env VR_SEG overrides (1..64)
     bool skip_enabled = true;
     unsigned long long* d_mask = nullptr;
@@ -139,6 +141,8 @@ vr_status build_frame(const vr_volume* vol, const vr_camera* cam, int W, int H, 
     P.seg_len = std::max(1, std::min(vol->seg_max, (int)((double)vol->seg_max / (double)step)));
     P.seg_span = (int)std::ceil((double)P.seg_len * (double)step) + 1;
     P.nbx = vol->NBX; P.nby = vol->NBY;
+    P.n_runs = vol->n_runs;
+    for (int k = 0; k < 2 * vr::MAX_RUNS; ++k) P.run_z[k] = vol->run_z[k];
     P.x_zero_below = table_zero_below(vol);   // the per-step opacity correction keeps zeros zero
 
     std::vector<vr::BrickPlan> plan;
@@ -247,13 +251,15 @@ vr_status launch_cast(vr_volume* vol, const Frame& f, int mode, float* d_img, un
     if (f.total_tiles == 0) return VR_OK;
     const int B = (int)f.recs.size();
     const bool skip = skip_applies(vol, mode) && vol->mask_valid;     // callers run ensure_mask first
-#define VR_LAUNCH(MODE_, SKIP_)                                                                              \
-    vr::cast_kernel<MODE_, INSTR, SKIP_><<<f.total_tiles, vr::CTA_THREADS, 0, vol->stream>>>(                \
+#define VR_LAUNCH(MODE_, SKIP_, CHAN_)                                                                       \
+    vr::cast_kernel<MODE_, INSTR, SKIP_, CHAN_><<<f.total_tiles, vr::CTA_THREADS, 0, vol->stream>>>(         \
         f.P, vol->d_bricks, B, vol->d_tiled, vol->d_tf_ea, vol->d_mask, d_img, d_counter, d_bitmap, d_mask_bitmap)
+    const bool chan = f.P.n_runs > 0;
     if (mode == VR_MODE_EA) {
-        if (skip) VR_LAUNCH(vr::MODE_EA, 1); else VR_LAUNCH(vr::MODE_EA, 0);
+        if (skip) { if (chan) VR_LAUNCH(vr::MODE_EA, 1, 1); else VR_LAUNCH(vr::MODE_EA, 1, 0); }
+        else { if (chan) VR_LAUNCH(vr::MODE_EA, 0, 1); else VR_LAUNCH(vr::MODE_EA, 0, 0); }
     } else {
-        VR_LAUNCH(vr::MODE_MIP, 0);
+        if (chan) VR_LAUNCH(vr::MODE_MIP, 0, 1); else VR_LAUNCH(vr::MODE_MIP, 0, 0);
     }
 #undef VR_LAUNCH
     VR_CUDA(cudaGetLastError(), "cast kernel launch");
@@ -416,6 +422,28 @@ vr_status vr_set_subcube(vr_volume* vol, const int lo[3], const int hi[3]) {
         if (lo[a] < 0 || hi[a] > vol->dims[a] || hi[a] < lo[a])
             return fail(VR_ERR_INVALID_ARG, "vr_set_subcube: need 0 <= lo_a <= hi_a <= n_a");
     for (int a = 0; a < 3; ++a) { vol->sub_lo[a] = lo[a]; vol->sub_hi[a] = hi[a]; }
+    return VR_OK;
+}
+
+vr_status vr_set_channel_mask(vr_volume* vol, const unsigned char* enabled) {
+    if (!vol) return fail(VR_ERR_INVALID_ARG, "vr_set_channel_mask: volume is NULL");
+    if (!enabled) { vol->n_runs = 0; return VR_OK; }                 // NULL: every channel enabled
+    static_assert(vr::MAX_RUNS == VR_MAX_CHANNEL_RUNS, "run limit of the kernels and of the header differ");
+    int runs[2 * vr::MAX_RUNS], n = 0;
+    const int nz = vol->dims[2];
+    for (int z = 0; z < nz;) {
+        if (!enabled[z]) { ++z; continue; }
+        int z1 = z;
+        while (z1 < nz && enabled[z1]) ++z1;
+        if (n == vr::MAX_RUNS)
+            return fail(VR_ERR_INVALID_ARG, "vr_set_channel_mask: more than VR_MAX_CHANNEL_RUNS runs of enabled channels");
+        runs[2 * n] = z; runs[2 * n + 1] = z1; ++n;
+        z = z1;
+    }
+    if (n == 1 && runs[0] == 0 && runs[1] == nz) { vol->n_runs = 0; return VR_OK; }   // all enabled = no mask
+    if (n == 0) { runs[0] = 0; runs[1] = 0; n = 1; }                 // nothing enabled: one empty run
+    vol->n_runs = n;
+    for (int k = 0; k < 2 * n; ++k) vol->run_z[k] = runs[k];
     return VR_OK;
 }
 

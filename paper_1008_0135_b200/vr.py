@@ -16,9 +16,10 @@ VR_OK, VR_ERR_INVALID_ARG, VR_ERR_STATE, VR_ERR_OOM, VR_ERR_CUDA = 0, 1, 2, 3, 4
 VR_MODE_EA, VR_MODE_MIP = 0, 1
 VR_PROJ_ORTHO, VR_PROJ_PERSP = 0, 1
 VR_MAX_BRICKS = 512
+VR_MAX_CHANNEL_RUNS = 16
 
 SYMBOLS = ["vr_create_volume", "vr_destroy_volume", "vr_set_stream", "vr_set_transfer_function",
-           "vr_set_bricks", "vr_set_subcube", "vr_render", "vr_render_to_host", "vr_render_bricks", "vr_composite",
+           "vr_set_bricks", "vr_set_subcube", "vr_set_channel_mask", "vr_render", "vr_render_to_host", "vr_render_bricks", "vr_composite",
            "vr_plan_bricks", "vr_measure", "vr_measure_units", "vr_set_empty_space_skipping", "vr_get_skip_info",
            "vr_set_l2_fetch_granularity",
            "vr_get_l2_fetch_granularity", "vr_get_stage_ms", "vr_volume_info", "vr_volume_range", "vr_export_linear", "vr_last_error"]
@@ -55,6 +56,7 @@ def lib():
         L.vr_set_transfer_function.argtypes = [vp, fp, C.c_float, C.c_float]
         L.vr_set_bricks.argtypes = [vp, C.c_int, C.c_int, C.c_int]
         L.vr_set_subcube.argtypes = [vp, ip, ip]
+        L.vr_set_channel_mask.argtypes = [vp, C.POINTER(C.c_ubyte)]
         L.vr_render.argtypes = [vp, cam, C.c_int, C.c_int, C.c_float, C.c_int, C.c_float, vp, vp]
         L.vr_render_to_host.argtypes = [vp, cam, C.c_int, C.c_int, C.c_float, C.c_int, C.c_float, vp]
         L.vr_render_bricks.argtypes = [vp, cam, C.c_int, C.c_int, C.c_float, C.c_int, C.c_float, vp]
@@ -184,6 +186,15 @@ class Volume:
             _check(lib().vr_set_subcube(self._h, None, None))
         else:
             _check(lib().vr_set_subcube(self._h, _i3(lo), _i3(hi)))
+
+    def vr_set_channel_mask(self, enabled=None):
+        """enabled: None (all channels) or nz values, non-zero = channel enabled."""
+        if enabled is None:
+            _check(lib().vr_set_channel_mask(self._h, None))
+            return
+        m = np.ascontiguousarray(np.asarray(enabled) != 0, dtype=np.uint8)
+        assert m.size == self.dims[2], "one value per spectral channel"
+        _check(lib().vr_set_channel_mask(self._h, m.ctypes.data_as(C.POINTER(C.c_ubyte))))
 
     def vr_render(self, cam, W, H, step, mode, ert_alpha=0.0, out=None, out_scalar=None):
         import torch

@@ -51,6 +51,7 @@ def test_null_and_range_checks_without_device(vr):
     assert L.vr_set_stream(None, None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_set_bricks(None, 1, 1, 1) == vr.VR_ERR_INVALID_ARG
     assert L.vr_set_subcube(None, None, None) == vr.VR_ERR_INVALID_ARG
+    assert L.vr_set_channel_mask(None, None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_set_transfer_function(None, None, 0.0, 1.0) == vr.VR_ERR_INVALID_ARG
     cam = vr.camera_from_spec(wl.orbit_camera((8, 8, 8), 30, 20, wl.PROJ_ORTHO))
     assert L.vr_render(None, C.byref(cam), 8, 8, 1.0, 0, 0.0, None, None) == vr.VR_ERR_INVALID_ARG
