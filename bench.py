@@ -112,6 +112,67 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+class NvmlSampler:
+    """The same clocks and throttle reasons read in-process through NVML (nvidia-ml-py) every 20 ms: no child process,
+    and many samples inside a timed region of ~0.2 s.  Falls back to ClockSampler (nvidia-smi) when NVML is missing."""
+    REASONS = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self.stop_flag = False
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(self._physical_index(index))
+            self.max_sm = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.fallback = ClockSampler(index)
+
+    @staticmethod
+    def _physical_index(index):
+        vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+        ids = [v for v in vis.split(",") if v.strip() != ""]
+        try:
+            return int(ids[index]) if ids else index
+        except (ValueError, IndexError):
+            return index
+
+    def start(self):
+        if not self.ok:
+            return self.fallback.start()
+        self.thread = threading.Thread(target=self._run, daemon=True)
+        self.thread.start()
+
+    def _run(self):
+        nv = self.nv
+        while not self.stop_flag:
+            try:
+                sm = float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    rs = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    rs = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                self.rows.append((time.time(), sm, rs))
+            except Exception:
+                pass
+            time.sleep(0.02)
+
+    def stop(self, t0, t1):
+        if not self.ok:
+            return self.fallback.stop(t0, t1)
+        self.stop_flag = True
+        self.thread.join(timeout=2)
+        rows = [r for r in self.rows if t0 <= r[0] <= t1] or self.rows
+        sm = [r[1] for r in rows]
+        reasons = sorted(n for n, bit in self.REASONS.items() if any(r[2] & bit for r in rows))
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": self.max_sm, "reasons": reasons,
+                "samples": len(sm), "source": "NVML in-process, 20 ms period, samples inside the timed region"}
+
+
 def workload_for(args):
     w = wl.config(args.config)
     if getattr(args, "image", None):
@@ -181,7 +242,7 @@ def run_ours(args):
     for k in range(Wm):
         frame(k)
     barrier()
-    sampler = ClockSampler(local)
+    sampler = NvmlSampler(local)
     if rank == 0:
         sampler.start()
     time.sleep(0.3)

@@ -16,6 +16,9 @@ namespace vr {
 
 constexpr int TILE = 8;                 // voxels per tile edge
 constexpr int TILE_ELEMS = 512;         // 8^3 floats = 2 KB, x-rows of 32 B = one DRAM sector
+// Padded coordinates of the tiled copy: u = voxel index + PAD.  y and z carry one replicated layer below index 0;
+// x carries a whole tile (8) so that the re-layout's row reads stay 32-byte aligned with the source rows.
+constexpr int PAD_X = 8, PAD_Y = 1, PAD_Z = 1;
 // CTA shape of the caster, chosen by measurement on the config-3 orbit (B200): 16x8 pixels (4 warps) with 7
 // CTAs per SM (72 registers) gave 5.88 ms mean cast time; 16x16 with 3 CTAs 6.08 ms; forcing 64 registers for
 // 8 CTAs (32 warps) 7.6 ms - more resident rays thrash the L1 that carries the sector re-use between rays.
@@ -65,11 +68,11 @@ struct BrickRec {
 };
 
 // ------------------------------------------------------------------------------------------------
-// a0  re-layout.  The tiled copy holds the cube in PADDED coordinates u = voxel index + 1: one replicated layer
-// below index 0 and at least one above index n-1 on every axis (T_a = ceil((n_a + 2)/8) tiles).  Trilinear
+// a0  re-layout.  The tiled copy holds the cube in PADDED coordinates u = voxel index + PAD_a (8, 1, 1): replicated
+// layers below index 0 and at least one above index n-1 on every axis (T_a = ceil((n_a + PAD_a + 1)/8) tiles).  Trilinear
 // interpolation between an edge voxel and its replica returns the edge value exactly (fma(f, v-v, v) = v), which is
 // O5's clamp-to-edge without a clamp, a floor of a negative number or a bounds test in the sample loop: a sample
-// at q = p - 1/2 in [-1/2, n - 1/2] reads padded cells floor(q + 1) in [0, n] and floor(q + 1) + 1 in [1, n + 1].
+// at q = p - 1/2 in [-1/2, n - 1/2] reads padded voxels floor(q) + PAD (>= PAD - 1) and floor(q) + PAD + 1 (<= n + PAD).
 // (An infinite voxel on a face would give inf - inf = NaN where the clamp gives inf; survey cubes blank with NaN.)
 // One CTA moves an 8(z) x 8(y) x 64(x) block: coalesced row reads -> shared memory -> 8 whole tiles written as
 // one contiguous 16 KB run of float4 stores.
@@ -100,13 +103,13 @@ relayout_kernel(const float* __restrict__ src, float* __restrict__ dst, int nx, 
     const int tx0 = blockIdx.x * 8, ty = blockIdx.y, tz = blockIdx.z;
     const int t = threadIdx.x;
     const int xo = t & 63;
-    const int xs = min(max(tx0 * 8 + xo - 1, 0), nx - 1);      // padded -> voxel, replicated at both ends
+    const int xs = min(max(tx0 * 8 + xo - PAD_X, 0), nx - 1);  // padded -> voxel, replicated at both ends
     float vmin = INFINITY, vmax = -INFINITY;
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
         const int row = (t >> 6) + 4 * k;
-        const int z = min(max(tz * 8 + (row >> 3) - 1, 0), nz - 1);
-        const int y = min(max(ty * 8 + (row & 7) - 1, 0), ny - 1);
+        const int z = min(max(tz * 8 + (row >> 3) - PAD_Z, 0), nz - 1);
+        const int y = min(max(ty * 8 + (row & 7) - PAD_Y, 0), ny - 1);
         const float val = __ldcs(src + ((size_t)z * ny + y) * nx + xs);
         sm[row][xo] = val;
         vmin = fminf(vmin, val);      // fminf/fmaxf ignore NaN (blanked voxels)
@@ -147,7 +150,7 @@ relayout_kernel(const float* __restrict__ src, float* __restrict__ dst, int nx, 
     }
 }
 
-// element offset of PADDED position (x,y,z) = voxel index + 1 in the tiled copy
+// element offset of PADDED position (x,y,z) = voxel index + (PAD_X, PAD_Y, PAD_Z) in the tiled copy
 __device__ __forceinline__ size_t tiled_index(int x, int y, int z, unsigned ty_stride, unsigned slab_stride) {
     return (size_t)(z >> 3) * slab_stride + (size_t)(y >> 3) * ty_stride + (size_t)(x >> 3) * TILE_ELEMS +
            (size_t)(((z & 7) << 6) | ((y & 7) << 3) | (x & 7));
@@ -161,7 +164,7 @@ __global__ void export_linear_kernel(const float* __restrict__ tiled, float* __r
         const int x = (int)(i % nx);
         const size_t r = i / nx;
         const int y = (int)(r % ny), z = (int)(r / ny);
-        dst[i] = tiled[tiled_index(x + 1, y + 1, z + 1, ty_stride, slab_stride)];
+        dst[i] = tiled[tiled_index(x + PAD_X, y + PAD_Y, z + PAD_Z, ty_stride, slab_stride)];
     }
 }
 
@@ -293,7 +296,7 @@ __device__ __forceinline__ void classify_blend(const float4* __restrict__ tf, co
 // ------------------------------------------------------------------------------------------------
 // NEXT-2  occupancy mask for empty-space skipping (PAPER.md:144 balanced work, PAPER.md:205 finding 2: the work
 // depends on the data, PAPER.md:294 noise-suppressing transfer functions).  One bit per PADDED cell (i,j,k), i in
-// [0, n_x] etc. = the unit cube between padded voxels i..i+1, j..j+1, k..k+1 in which O5 interpolates (cell 0 and
+// [0, n_x + PAD_X) etc. = the unit cube between padded voxels i..i+1, j..j+1, k..k+1 in which O5 interpolates (cell 0 and
 // cell n_a are the half-voxel rims where the replicated layer stands in for the clamp).  The bit is CLEAR when
 // every sample in the cell contributes exactly nothing under the current table:
 //   * a corner is NaN  -> the blend is NaN -> the sample is skipped (O5/A14), or
@@ -317,7 +320,7 @@ build_mask_kernel(const float* __restrict__ vol, unsigned ty_stride, unsigned sl
     if (t < 64) (&words[0][0][0][0])[t] = 0u;
     for (int i = t; i < 9 * 9 * 33; i += 256) {
         const int lx = i % 33, r = i / 33, ly = r % 9, lz = r / 9;
-        const int x = min(x0 + lx, nx + 1), y = min(y0 + ly, ny + 1), z = min(z0 + lz, nz + 1);   // padded coordinates
+        const int x = min(x0 + lx, nx + PAD_X), y = min(y0 + ly, ny + PAD_Y), z = min(z0 + lz, nz + PAD_Z);   // padded coordinates
         const float v = __ldg(vol + tiled_index(x, y, z, ty_stride, slab_stride));
         const float xt = __saturatef((v - vmin) * inv_range) * 255.0f;
         cls[lz][ly][lx] = (v != v) ? 2 : (xt < x_zero_below - MASK_MARGIN ? 0 : 1);
@@ -330,7 +333,7 @@ build_mask_kernel(const float* __restrict__ vol, unsigned ty_stride, unsigned sl
         const int lx = lxq + k;
         const unsigned o = cls[lz][ly][lx] | cls[lz][ly][lx + 1] | cls[lz][ly + 1][lx] | cls[lz][ly + 1][lx + 1] |
                            cls[lz + 1][ly][lx] | cls[lz + 1][ly][lx + 1] | cls[lz + 1][ly + 1][lx] | cls[lz + 1][ly + 1][lx + 1];
-        const bool in = (x0 + lx <= nx) && (y0 + ly <= ny) && (z0 + lz <= nz);      // n_a + 1 cells per axis
+        const bool in = (x0 + lx < nx + PAD_X) && (y0 + ly < ny + PAD_Y) && (z0 + lz < nz + PAD_Z);   // n_a + PAD_a padded cells per axis
         if (in && (o & 1u) && !(o & 2u)) bits |= 1u << k;
     }
     // bits 0..3 -> word wx = 2*(t&3), bits 4..7 -> word wx + 1; bit position in the word: (lz&3)*16 + (ly&3)*4 + lx&3
@@ -343,7 +346,7 @@ build_mask_kernel(const float* __restrict__ vol, unsigned ty_stride, unsigned sl
         const int wx = t & 7, wyy = (t >> 3) & 1, wzz = t >> 4;
         const int bx = blockIdx.x * 8 + wx, by = blockIdx.y * 2 + wyy, bz = blockIdx.z * 2 + wzz;
         const unsigned long long w = (unsigned long long)words[wzz][wyy][wx][0] | ((unsigned long long)words[wzz][wyy][wx][1] << 32);
-        const bool in = bx < NBX && by < NBY && bz * 4 <= nz;
+        const bool in = bx < NBX && by < NBY && bz * 4 < nz + PAD_Z;
         if (in) mask[((size_t)bz * NBY + by) * NBX + bx] = w;
         unsigned long long cnt = in ? (unsigned long long)__popcll(w) : 0ull;
         for (int sft = 16; sft > 0; sft >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, sft);

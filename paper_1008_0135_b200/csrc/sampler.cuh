@@ -58,7 +58,7 @@ __device__ __forceinline__ const float* elem_ptr(unsigned long long base, unsign
 }
 
 // Segment anchor: integer origin and remainder of the segment's first sample, in PADDED coordinates
-// u = q + 1 = p + 1/2 (kernels.cuh, re-layout): no clamp is needed, the replicated layers do O5's clamp-to-edge.
+// u = q + PAD = p - 1/2 + PAD (kernels.cuh, re-layout): no clamp is needed, the replicated layers do O5's clamp-to-edge.
 struct Anchor {
     int O[3];
     float rel[3];
@@ -72,7 +72,7 @@ __device__ __forceinline__ void set_anchor(const double o[3], const double d[3],
     const double ta = t_near + ((double)i0 + 0.5) * step;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-        const double ud = o[a] + ta * d[a] + 0.5;
+        const double ud = o[a] + ta * d[a] + ((a == 0 ? PAD_X : a == 1 ? PAD_Y : PAD_Z) - 0.5);
         const double base = floor(ud) - (h[a] < 0.0f ? (double)span : 0.0);
         A.O[a] = (int)base;
         A.rel[a] = (float)(ud - base);

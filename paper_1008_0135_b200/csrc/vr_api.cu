@@ -224,7 +224,7 @@ vr_status ensure_mask(vr_volume* vol) {
     if (e == cudaSuccess) e = cudaMemsetAsync(vol->d_mask_count, 0, sizeof(unsigned long long), vol->stream);
     if (e == cudaSuccess) e = cudaEventRecord(e0, vol->stream);
     if (e == cudaSuccess) {
-        dim3 grid((vol->dims[0] + 1 + 31) / 32, (vol->dims[1] + 1 + 7) / 8, (vol->dims[2] + 1 + 7) / 8);
+        dim3 grid((vol->dims[0] + vr::PAD_X + 31) / 32, (vol->dims[1] + vr::PAD_Y + 7) / 8, (vol->dims[2] + vr::PAD_Z + 7) / 8);
         vr::build_mask_kernel<<<grid, 256, 0, vol->stream>>>(
             vol->d_tiled, (unsigned)vol->TX * vr::TILE_ELEMS, (unsigned)vol->TX * (unsigned)vol->TY * vr::TILE_ELEMS,
             vol->dims[0], vol->dims[1], vol->dims[2], key[0], key[1], key[2], vol->d_mask, vol->NBX, vol->NBY,
@@ -280,10 +280,14 @@ vr_status launch_composite(vr_volume* vol, const Frame& f, int mode, const float
     return VR_OK;
 }
 
-vr_status ensure_pool(vr_volume* vol, size_t floats) {
+// Brick images of vr_render live in one grow-only pool.  The rectangles change with the view, so the request is
+// rounded up to the most a frame of this size can need (every brick a full frame) when that is modest (<= 1 GiB),
+// else doubled: a camera orbit then never reallocates inside a frame sequence (cudaFree synchronises the device).
+vr_status ensure_pool(vr_volume* vol, size_t floats, size_t full_frames_floats = 0) {
     if (floats <= vol->pool_floats) return VR_OK;
     if (vol->d_pool) { cudaFree(vol->d_pool); vol->d_pool = nullptr; vol->pool_floats = 0; }
-    const size_t want = floats + floats / 4;
+    size_t want = floats * 2;
+    if (full_frames_floats >= floats && full_frames_floats * sizeof(float) <= ((size_t)1 << 30)) want = full_frames_floats;
     VR_CUDA(cudaMalloc(&vol->d_pool, want * sizeof(float)), "allocate brick images");
     vol->pool_floats = want;
     return VR_OK;
@@ -307,13 +311,14 @@ vr_status vr_create_volume(const int dims[3], const float* d_data, vr_volume** o
         const int sv = std::atoi(e_);
         if (sv >= 1 && sv <= 64) v->seg_max = sv;
     }
-    v->TX = (dims[0] + 2 + 7) / 8; v->TY = (dims[1] + 2 + 7) / 8; v->TZ = (dims[2] + 2 + 7) / 8;   // padded: +1 layer each side
+    // padded: PAD_a replicated layers below, at least one above
+    v->TX = (dims[0] + vr::PAD_X + 1 + 7) / 8; v->TY = (dims[1] + vr::PAD_Y + 1 + 7) / 8; v->TZ = (dims[2] + vr::PAD_Z + 1 + 7) / 8;
     if ((double)v->TX * v->TY * vr::TILE_ELEMS >= 1073741824.0) {   // slab bytes and in-slab offsets stay 32-bit
         delete v;
         return fail(VR_ERR_INVALID_ARG, "vr_create_volume: nx*ny too large for 32-bit in-slab offsets");
     }
     v->tiled_elems = (size_t)v->TX * v->TY * v->TZ * vr::TILE_ELEMS;
-    v->NBX = (dims[0] + 1 + 3) / 4; v->NBY = (dims[1] + 1 + 3) / 4; v->NBZ = (dims[2] + 1 + 3) / 4;   // n_a + 1 padded cells
+    v->NBX = (dims[0] + vr::PAD_X + 3) / 4; v->NBY = (dims[1] + vr::PAD_Y + 3) / 4; v->NBZ = (dims[2] + vr::PAD_Z + 3) / 4;   // n_a + PAD_a padded cells
     v->mask_words = (size_t)v->NBX * v->NBY * v->NBZ;
     cudaError_t e = cudaMalloc(&v->d_tiled, v->tiled_elems * sizeof(float));
     if (e == cudaSuccess) e = cudaMalloc(&v->d_range, 2 * vr::RANGE_SLOTS * sizeof(unsigned));
@@ -459,7 +464,8 @@ vr_status vr_render(vr_volume* vol, const vr_camera* cam, int W, int H, float st
     if ((s = upload_plan(vol, f)) != VR_OK) return s;
     if (mode == VR_MODE_EA && (s = upload_tf_for_step(vol, (double)step)) != VR_OK) return s;
     vol->timed_cast = vol->timed_comp = false;
-    if (!direct && (s = ensure_pool(vol, f.pool_pixels * (mode == VR_MODE_EA ? 4 : 1))) != VR_OK) return s;
+    if (!direct && (s = ensure_pool(vol, f.pool_pixels * (mode == VR_MODE_EA ? 4 : 1),
+                                    (size_t)B * W * H * (mode == VR_MODE_EA ? 4 : 1))) != VR_OK) return s;
     if (skip_applies(vol, mode) && (s = ensure_mask(vol)) != VR_OK) return s;   // builds only after a table change
     VR_CUDA(cudaEventRecord(vol->ev[0], vol->stream), "record event");
     s = launch_cast<0>(vol, f, mode, direct ? d_out_rgba : vol->d_pool, nullptr, nullptr, nullptr);

@@ -131,7 +131,7 @@ def test_full_size_ortho_sample_count_law(vr, gass):
     V = float(w.dims[0]) * w.dims[1] * w.dims[2]
     p = 2.0 * cs.ortho_half_h / 1024.0
     assert abs(samples / (V / (p * p)) - 1.0) < 0.01
-    total_sectors = (-(-(w.dims[0] + 2) // 8)) * (-(-(w.dims[1] + 2) // 8)) * (-(-(w.dims[2] + 2) // 8)) * 64
+    total_sectors = (-(-(w.dims[0] + 9) // 8)) * (-(-(w.dims[1] + 2) // 8)) * (-(-(w.dims[2] + 2) // 8)) * 64
     assert 0.5 * total_sectors < sectors <= total_sectors
 
 

@@ -270,21 +270,22 @@ def test_measure_counts_every_sample_once(vr, oracle):
         vol.close()
         ref = oracle.render(cube.cpu().numpy(), tab, -3.0, 8.0, bricks, ocam(oracle, cs), W, H, 0.5, 0, 0.0, route=1)
         assert samples == ref["samples"]
-        total_sectors = -(-72 // 8) * -(-47 // 8) * -(-54 // 8) * 64
+        total_sectors = -(-79 // 8) * -(-47 // 8) * -(-54 // 8) * 64
         assert 0 < sectors <= total_sectors
 
 
 def _footprint_units(oracle, dims, cs, W, H, step, eps):
-    """Distinct 32/64/128-byte units of the tiled cube (padded coordinates u = voxel + 1
-    with one replicated layer on each side, 8^3 tiles, T_a = ceil((n_a+2)/8), element index
+    """Distinct 32/64/128-byte units of the tiled cube (padded coordinates u = voxel + PAD,
+    PAD = (8, 1, 1), replicated layers on each side, 8^3 tiles, T_a = ceil((n_a+PAD_a+1)/8), element index
     ((tz*TY + ty)*TX + tx)*512 + lz*64 + ly*8 + lx of (ux,uy,uz), sector = index >> 3) touched by the 2x2x2
-    footprints (u0, u0+1 per axis, u0 = floor(p + 1/2)) of the ORACLE's sample positions
+    footprints (u0, u0+1 per axis, u0 = floor(p - 1/2 + PAD)) of the ORACLE's sample positions
     t_i = t_near + (i + 1/2) step, enumerated here in numpy.  Returns (must, may): `must` counts only footprints
     whose floor is the same for any position error below eps voxels, `may` adds both candidates of the others —
     the GPU computes positions in fp32 (error ~1e-5 voxel at these sizes), so its count lies in [must, may]."""
     nx, ny, nz = dims
     n_a = np.array([nx, ny, nz])
-    TX, TY = (nx + 9) // 8, (ny + 9) // 8
+    TX, TY = (nx + 16) // 8, (ny + 9) // 8
+    pad = np.array([8, 1, 1])
     cam = oracle.make_camera(cs.view, cs.projection, cs.fovy_deg, cs.ortho_half_h)
     must, may = [], []
     for py in range(H):
@@ -294,11 +295,11 @@ def _footprint_units(oracle, dims, cs, W, H, step, eps):
             if n == 0:
                 continue
             t = tn + (np.arange(n) + 0.5) * step
-            q = o[None, :] + t[:, None] * d[None, :] + 0.5          # padded coordinates, in [1/2, n + 1/2]
+            q = o[None, :] + t[:, None] * d[None, :] - 0.5 + pad[None, :]   # padded coordinates, in [PAD - 1/2, n + PAD - 1/2]
             i0 = np.floor(q).astype(np.int64)
             f = q - i0
-            lo_amb = (f < eps) & (i0 > 0)                       # could floor to i0 - 1
-            hi_amb = (f > 1.0 - eps) & (i0 < n_a[None, :])      # could floor to i0 + 1
+            lo_amb = (f < eps) & (i0 > (pad - 1)[None, :])      # could floor to i0 - 1
+            hi_amb = (f > 1.0 - eps) & (i0 < (n_a + pad - 1)[None, :])  # could floor to i0 + 1
             for shift, dest in ((0, must), (-1, None), (1, None)):
                 for corner in range(8):
                     c = np.array([(corner >> a) & 1 for a in range(3)])
@@ -341,7 +342,7 @@ def test_measure_sector_count_equals_numpy_enumeration(vr, oracle, proj, bricks,
     assert evaluated == samples and e3 == s3 and units[3] == 0     # tf_ramp has alpha > 0 from entry 1: no skipping
     units, units_mip = units[:3], units_mip[:3]
     must, may, _ = _footprint_units(oracle, dims, cs, W, H, step, eps=2e-4)
-    total = ((70 + 9) // 8) * ((45 + 9) // 8) * ((52 + 9) // 8) * 64
+    total = ((70 + 16) // 8) * ((45 + 9) // 8) * ((52 + 9) // 8) * 64
     print(f"sectors gpu {units} numpy must {must} may {may} of {total}")
     assert sectors == units[0] and s2 == samples == s3 and units_mip == units
     assert must[0] < 0.92 * total                          # sparse enough to be a test
