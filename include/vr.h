@@ -187,6 +187,12 @@ vr_status vr_volume_info(const vr_volume* vol, float* h_relayout_ms, long long* 
  *     give one ("each GPU computes the minimum and maximum of its portion").
  *     STATE if every voxel is NaN.                                                               */
 vr_status vr_volume_range(const vr_volume* vol, float* h_min, float* h_max);
+/* Histogram of the cube's voxels (the data range — and with it the colour map and the threshold
+ *     of a noise-suppressing table, PAPER.md:294 — is chosen from the data).  n_bins (1..4096) equal bins over
+ *     [lo, hi): bin = floor((v - lo) * (n_bins / (hi - lo))) evaluated in float32, values outside the range are
+ *     counted in the first / last bin, NaN voxels only in *h_nan (may be NULL).  h_counts: HOST, n_bins entries.
+ *     One streaming pass over the tiled copy; synchronises.  INVALID_ARG: NULL, n_bins out of range, lo >= hi.     */
+vr_status vr_volume_histogram(vr_volume* vol, int n_bins, float lo, float hi, long long* h_counts, long long* h_nan);
 /* Inverse of the re-layout: gathers the tiled copy back into d_linear[nz][ny][nx] (round-trip test). */
 vr_status vr_export_linear(vr_volume* vol, float* d_linear);
 

@@ -156,6 +156,43 @@ __device__ __forceinline__ size_t tiled_index(int x, int y, int z, unsigned ty_s
            (size_t)(((z & 7) << 6) | ((y & 7) << 3) | (x & 7));
 }
 
+// NEXT-1  histogram of the cube (the data range and distribution the colour map is built on).
+// One pass over the tiled copy; padding replicas are not counted.  bin = floor((v - lo) * scale) in fp32, clamped to
+// [0, n_bins - 1]; NaN voxels are counted in nan_count only.  Per-CTA shared-memory bins, then one global add per bin.
+constexpr int HIST_MAX_BINS = 4096;
+__global__ void __launch_bounds__(256)
+histogram_kernel(const float* __restrict__ tiled, size_t n_tiles, int TX, int TY, int nx, int ny, int nz, float lo,
+                 float scale, int n_bins, unsigned long long* __restrict__ bins, unsigned long long* __restrict__ nan_count) {
+    extern __shared__ unsigned sh_bins[];
+    for (int i = threadIdx.x; i < n_bins; i += 256) sh_bins[i] = 0u;
+    __syncthreads();
+    unsigned nans = 0;
+    for (size_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const int tx = (int)(tile % TX), ty = (int)((tile / TX) % TY), tz = (int)(tile / ((size_t)TX * TY));
+        const float4* src = reinterpret_cast<const float4*>(tiled + tile * TILE_ELEMS);
+        for (int q = threadIdx.x; q < TILE_ELEMS / 4; q += 256) {
+            const float4 v4 = __ldcs(src + q);
+            const int lx = (q & 1) * 4, ly = (q >> 1) & 7, lz = q >> 4;
+            const int y = ty * 8 + ly - PAD_Y, z = tz * 8 + lz - PAD_Z;
+            if (y < 0 || y >= ny || z < 0 || z >= nz) continue;
+            const float v[4] = {v4.x, v4.y, v4.z, v4.w};
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int x = tx * 8 + lx + k - PAD_X;
+                if (x < 0 || x >= nx) continue;
+                if (v[k] != v[k]) { ++nans; continue; }
+                const float b = floorf((v[k] - lo) * scale);
+                const int bi = (int)fminf(fmaxf(b, 0.0f), (float)(n_bins - 1));
+                atomicAdd(&sh_bins[bi], 1u);
+            }
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < n_bins; i += 256)
+        if (sh_bins[i]) atomicAdd(&bins[i], (unsigned long long)sh_bins[i]);
+    if (nans) atomicAdd(nan_count, (unsigned long long)nans);
+}
+
 // inverse of a0 (round-trip test only)
 __global__ void export_linear_kernel(const float* __restrict__ tiled, float* __restrict__ dst, int nx, int ny,
                                      int nz, unsigned ty_stride, unsigned slab_stride) {

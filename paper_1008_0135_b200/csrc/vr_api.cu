@@ -665,6 +665,33 @@ vr_status vr_volume_range(const vr_volume* vol, float* h_min, float* h_max) {
     return VR_OK;
 }
 
+vr_status vr_volume_histogram(vr_volume* vol, int n_bins, float lo, float hi, long long* h_counts, long long* h_nan) {
+    if (!vol || !h_counts) return fail(VR_ERR_INVALID_ARG, "vr_volume_histogram: NULL argument");
+    if (n_bins < 1 || n_bins > vr::HIST_MAX_BINS) return fail(VR_ERR_INVALID_ARG, "vr_volume_histogram: n_bins must be in [1,4096]");
+    if (!std::isfinite(lo) || !std::isfinite(hi) || !(hi > lo)) return fail(VR_ERR_INVALID_ARG, "vr_volume_histogram: need finite lo < hi");
+    unsigned long long* d_bins = nullptr;
+    VR_CUDA(cudaMalloc(&d_bins, (size_t)(n_bins + 1) * sizeof(unsigned long long)), "allocate histogram");
+    cudaError_t e = cudaMemsetAsync(d_bins, 0, (size_t)(n_bins + 1) * sizeof(unsigned long long), vol->stream);
+    std::vector<unsigned long long> h((size_t)n_bins + 1, 0ull);
+    if (e == cudaSuccess) {
+        const size_t n_tiles = (size_t)vol->TX * vol->TY * vol->TZ;
+        const float scale = (float)n_bins / (hi - lo);
+        // one CTA covers many tiles; sub-2^32 counts per CTA bin: at most n_tiles/grid * 512 voxels per CTA
+        const int grid = (int)std::min<size_t>(n_tiles, 148 * 8);
+        vr::histogram_kernel<<<grid, 256, (size_t)n_bins * sizeof(unsigned), vol->stream>>>(
+            vol->d_tiled, n_tiles, vol->TX, vol->TY, vol->dims[0], vol->dims[1], vol->dims[2], lo, scale, n_bins, d_bins,
+            d_bins + n_bins);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h.data(), d_bins, h.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost, vol->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(vol->stream);
+    cudaFree(d_bins);
+    if (e != cudaSuccess) return cuda_fail(e, "vr_volume_histogram");
+    for (int i = 0; i < n_bins; ++i) h_counts[i] = (long long)h[i];
+    if (h_nan) *h_nan = (long long)h[n_bins];
+    return VR_OK;
+}
+
 vr_status vr_export_linear(vr_volume* vol, float* d_linear) {
     if (!vol || !d_linear) return fail(VR_ERR_INVALID_ARG, "vr_export_linear: NULL argument");
     vr::export_linear_kernel<<<1184, 256, 0, vol->stream>>>(vol->d_tiled, d_linear, vol->dims[0], vol->dims[1],

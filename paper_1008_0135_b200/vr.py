@@ -22,7 +22,7 @@ SYMBOLS = ["vr_create_volume", "vr_destroy_volume", "vr_set_stream", "vr_set_tra
            "vr_set_bricks", "vr_set_subcube", "vr_set_channel_mask", "vr_render", "vr_render_to_host", "vr_render_bricks", "vr_composite",
            "vr_plan_bricks", "vr_measure", "vr_measure_units", "vr_set_empty_space_skipping", "vr_get_skip_info",
            "vr_set_l2_fetch_granularity",
-           "vr_get_l2_fetch_granularity", "vr_get_stage_ms", "vr_volume_info", "vr_volume_range", "vr_export_linear", "vr_last_error"]
+           "vr_get_l2_fetch_granularity", "vr_get_stage_ms", "vr_volume_info", "vr_volume_range", "vr_volume_histogram", "vr_export_linear", "vr_last_error"]
 
 
 class vr_camera(C.Structure):
@@ -73,6 +73,7 @@ def lib():
         L.vr_get_stage_ms.argtypes = [vp, fp, fp]
         L.vr_volume_info.argtypes = [vp, fp, C.POINTER(C.c_longlong)]
         L.vr_volume_range.argtypes = [vp, fp, fp]
+        L.vr_volume_histogram.argtypes = [vp, C.c_int, C.c_float, C.c_float, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
         L.vr_export_linear.argtypes = [vp, vp]
         L.vr_last_error.argtypes = []
         L.vr_last_error.restype = C.c_char_p
@@ -268,6 +269,14 @@ class Volume:
         a, b = C.c_float(0), C.c_float(0)
         _check(lib().vr_volume_range(self._h, C.byref(a), C.byref(b)))
         return a.value, b.value
+
+    def vr_volume_histogram(self, n_bins, lo, hi):
+        """(counts [n_bins] int64, number of NaN voxels); outliers fall into the end bins."""
+        counts = np.zeros(int(n_bins), dtype=np.int64)
+        nan = C.c_longlong(0)
+        _check(lib().vr_volume_histogram(self._h, int(n_bins), float(lo), float(hi),
+                                         counts.ctypes.data_as(C.POINTER(C.c_longlong)), C.byref(nan)))
+        return counts, nan.value
 
     def vr_export_linear(self):
         import torch

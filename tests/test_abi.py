@@ -65,6 +65,7 @@ def test_null_and_range_checks_without_device(vr):
     assert L.vr_volume_info(None, None, None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_export_linear(None, None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_volume_range(None, None, None) == vr.VR_ERR_INVALID_ARG
+    assert L.vr_volume_histogram(None, 16, 0.0, 1.0, None, None) == vr.VR_ERR_INVALID_ARG
     L.vr_destroy_volume(None)     # no-op
 
 

@@ -373,6 +373,28 @@ def test_volume_range_equals_library_min_max(vr):
     vol.close()
 
 
+def test_volume_histogram_equals_numpy(vr):
+    """NEXT-1: histogram of the voxels = numpy's count of the same float32 bin expression, bit
+    for bit; padding replicas are not counted, NaN voxels are reported apart, outliers land in the end bins."""
+    import torch
+    for dims, seed, bins in [((61, 35, 19), 1, 64), ((130, 70, 33), 5, 1000), ((8, 8, 8), 2, 1), ((200, 9, 3), 4, 4096)]:
+        g = torch.Generator(device="cuda").manual_seed(seed)
+        cube = torch.randn((dims[2], dims[1], dims[0]), generator=g, device="cuda") * 3.0 + 1.0
+        cube[0, 0, 0] = float("nan")
+        vol = vr.Volume(cube)
+        lo, hi = -4.0, 7.5
+        counts, n_nan = vol.vr_volume_histogram(bins, lo, hi)
+        vol.close()
+        v = cube.cpu().numpy().reshape(-1)
+        ok = ~np.isnan(v)
+        scale = np.float32(bins) / (np.float32(hi) - np.float32(lo))
+        b = np.floor((v[ok] - np.float32(lo)) * scale)
+        b = np.clip(b, 0, bins - 1).astype(np.int64)
+        want = np.bincount(b, minlength=bins)
+        assert n_nan == 1 and counts.sum() == v.size - 1
+        assert np.array_equal(counts, want), (dims, bins)
+
+
 def test_subcube_and_channel_range_match_oracle(vr, oracle):
     """NEXT-3 / S1: sub-cube and spectral-channel selection, GPU vs oracle, bricked and not."""
     import torch
