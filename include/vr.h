@@ -130,11 +130,18 @@ vr_status vr_get_skip_info(vr_volume* vol, int* h_active, float* h_build_ms, lon
 vr_status vr_render(vr_volume* vol, const vr_camera* cam, int W, int H, float step_voxels, int mode,
                     float ert_alpha, float* d_out_rgba, float* d_out_scalar);
 
-/* Same frame delivered to HOST memory: vr_render into an internal device frame, then a
- *     device->host copy of it into h_out_rgba (H*W*4 floats; pinned memory makes the copy
- *     asynchronous) and a stream synchronisation.  This is the end-to-end call bench.py times. */
+/* Same frame delivered to HOST memory (the frame is returned to the viewer): vr_render into an
+ *     internal device frame, then a device->host copy of it into h_out_rgba (H*W*4 floats; pinned memory makes the
+ *     copy asynchronous), then a wait for that copy.  This is the end-to-end call bench.py times.
+ * vr_render_to_host_async: the same without the wait.  Two internal device frames are used alternately and the
+ *     copy runs on a stream of its own, so the copy of frame k overlaps the ray casting of frame k+1; the caller
+ *     keeps h_out_rgba untouched until vr_wait_frames (which waits for every copy issued so far) and uses a
+ *     different host buffer for the next frame.                                                                */
 vr_status vr_render_to_host(vr_volume* vol, const vr_camera* cam, int W, int H, float step_voxels,
                             int mode, float ert_alpha, float* h_out_rgba);
+vr_status vr_render_to_host_async(vr_volume* vol, const vr_camera* cam, int W, int H, float step_voxels,
+                                  int mode, float ert_alpha, float* h_out_rgba);
+vr_status vr_wait_frames(vr_volume* vol);
 
 /* Inspection level (the paper's two stages taken apart):
  * vr_render_bricks: steps a1-a5 only.  d_brick_images: DEVICE, caller-owned, B*H*W*4 floats (EA:

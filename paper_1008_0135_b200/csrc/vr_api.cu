@@ -60,8 +60,11 @@ struct vr_volume {
 
     float* d_pool = nullptr;          // rect-cropped brick images of vr_render
     size_t pool_floats = 0;
-    float* d_frame = nullptr;         // internal frame of vr_render_to_host
+    float* d_frame[2] = {nullptr, nullptr};   // internal frames of vr_render_to_host(_async), used alternately
     size_t frame_floats = 0;
+    cudaStream_t copy_stream = nullptr;        // device->host copies of finished frames
+    cudaEvent_t frame_done[2] = {nullptr, nullptr}, copy_done[2] = {nullptr, nullptr};
+    unsigned frame_idx = 0;
 
     // NEXT-2 empty-space skipping: occupancy mask (one bit per voxel cell), built for the current table on demand
     int n_runs = 0;                   // S2 channel mask as runs of enabled channels; 0 = every channel enabled
@@ -376,7 +379,12 @@ void vr_destroy_volume(vr_volume* v) {
     if (v->d_bricks) cudaFree(v->d_bricks);
     if (v->d_order) cudaFree(v->d_order);
     if (v->d_pool) cudaFree(v->d_pool);
-    if (v->d_frame) cudaFree(v->d_frame);
+    for (int k = 0; k < 2; ++k) {
+        if (v->d_frame[k]) cudaFree(v->d_frame[k]);
+        if (v->frame_done[k]) cudaEventDestroy(v->frame_done[k]);
+        if (v->copy_done[k]) cudaEventDestroy(v->copy_done[k]);
+    }
+    if (v->copy_stream) cudaStreamDestroy(v->copy_stream);
     if (v->d_mask) cudaFree(v->d_mask);
     if (v->d_mask_count) cudaFree(v->d_mask_count);
     for (int k = 0; k < 4; ++k)
@@ -493,23 +501,53 @@ vr_status vr_get_stage_ms(vr_volume* vol, float* h_cast_ms, float* h_composite_m
     return VR_OK;
 }
 
-vr_status vr_render_to_host(vr_volume* vol, const vr_camera* cam, int W, int H, float step, int mode, float ert,
-                            float* h_out_rgba) {
+vr_status vr_render_to_host_async(vr_volume* vol, const vr_camera* cam, int W, int H, float step, int mode, float ert,
+                                  float* h_out_rgba) {
     if (!h_out_rgba) return fail(VR_ERR_INVALID_ARG, "vr_render_to_host: h_out_rgba is NULL");
     if (!vol) return fail(VR_ERR_INVALID_ARG, "volume is NULL");
     if (W <= 0 || H <= 0 || W > 32768 || H > 32768) return fail(VR_ERR_INVALID_ARG, "W and H must be in [1,32768]");
     const size_t floats = (size_t)W * H * 4;
+    if (!vol->copy_stream) {
+        VR_CUDA(cudaStreamCreateWithFlags(&vol->copy_stream, cudaStreamNonBlocking), "create copy stream");
+        for (int k = 0; k < 2; ++k) {
+            VR_CUDA(cudaEventCreateWithFlags(&vol->frame_done[k], cudaEventDisableTiming), "create event");
+            VR_CUDA(cudaEventCreateWithFlags(&vol->copy_done[k], cudaEventDisableTiming), "create event");
+        }
+    }
     if (floats > vol->frame_floats) {
-        if (vol->d_frame) { cudaFree(vol->d_frame); vol->d_frame = nullptr; vol->frame_floats = 0; }
-        VR_CUDA(cudaMalloc(&vol->d_frame, floats * sizeof(float)), "allocate frame");
+        VR_CUDA(cudaStreamSynchronize(vol->copy_stream), "vr_render_to_host");       // no copy may be reading a frame
+        for (int k = 0; k < 2; ++k) {
+            if (vol->d_frame[k]) { cudaFree(vol->d_frame[k]); vol->d_frame[k] = nullptr; }
+        }
+        vol->frame_floats = 0;
+        for (int k = 0; k < 2; ++k) VR_CUDA(cudaMalloc(&vol->d_frame[k], floats * sizeof(float)), "allocate frame");
         vol->frame_floats = floats;
     }
-    vr_status s = vr_render(vol, cam, W, H, step, mode, ert, vol->d_frame, nullptr);
+    const int slot = (int)(vol->frame_idx & 1u);
+    // the copy that last read this device frame must be over before the compositor overwrites it
+    if (vol->frame_idx >= 2) VR_CUDA(cudaStreamWaitEvent(vol->stream, vol->copy_done[slot], 0), "wait for copy");
+    vr_status s = vr_render(vol, cam, W, H, step, mode, ert, vol->d_frame[slot], nullptr);
     if (s != VR_OK) return s;
-    VR_CUDA(cudaMemcpyAsync(h_out_rgba, vol->d_frame, floats * sizeof(float), cudaMemcpyDeviceToHost, vol->stream),
+    VR_CUDA(cudaEventRecord(vol->frame_done[slot], vol->stream), "record event");
+    VR_CUDA(cudaStreamWaitEvent(vol->copy_stream, vol->frame_done[slot], 0), "wait for frame");
+    VR_CUDA(cudaMemcpyAsync(h_out_rgba, vol->d_frame[slot], floats * sizeof(float), cudaMemcpyDeviceToHost, vol->copy_stream),
             "copy frame to host");
-    VR_CUDA(cudaStreamSynchronize(vol->stream), "vr_render_to_host");
+    VR_CUDA(cudaEventRecord(vol->copy_done[slot], vol->copy_stream), "record event");
+    ++vol->frame_idx;
     return VR_OK;
+}
+
+vr_status vr_wait_frames(vr_volume* vol) {
+    if (!vol) return fail(VR_ERR_INVALID_ARG, "vr_wait_frames: volume is NULL");
+    if (vol->copy_stream) VR_CUDA(cudaStreamSynchronize(vol->copy_stream), "vr_wait_frames");
+    return VR_OK;
+}
+
+vr_status vr_render_to_host(vr_volume* vol, const vr_camera* cam, int W, int H, float step, int mode, float ert,
+                            float* h_out_rgba) {
+    vr_status s = vr_render_to_host_async(vol, cam, W, H, step, mode, ert, h_out_rgba);
+    if (s != VR_OK) return s;
+    return vr_wait_frames(vol);
 }
 
 vr_status vr_render_bricks(vr_volume* vol, const vr_camera* cam, int W, int H, float step, int mode, float ert,

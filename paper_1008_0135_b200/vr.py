@@ -19,7 +19,7 @@ VR_MAX_BRICKS = 512
 VR_MAX_CHANNEL_RUNS = 16
 
 SYMBOLS = ["vr_create_volume", "vr_destroy_volume", "vr_set_stream", "vr_set_transfer_function",
-           "vr_set_bricks", "vr_set_subcube", "vr_set_channel_mask", "vr_render", "vr_render_to_host", "vr_render_bricks", "vr_composite",
+           "vr_set_bricks", "vr_set_subcube", "vr_set_channel_mask", "vr_render", "vr_render_to_host", "vr_render_to_host_async", "vr_wait_frames", "vr_render_bricks", "vr_composite",
            "vr_plan_bricks", "vr_measure", "vr_measure_units", "vr_set_empty_space_skipping", "vr_get_skip_info",
            "vr_set_l2_fetch_granularity",
            "vr_get_l2_fetch_granularity", "vr_get_stage_ms", "vr_volume_info", "vr_volume_range", "vr_volume_histogram", "vr_export_linear", "vr_last_error"]
@@ -59,6 +59,8 @@ def lib():
         L.vr_set_channel_mask.argtypes = [vp, C.POINTER(C.c_ubyte)]
         L.vr_render.argtypes = [vp, cam, C.c_int, C.c_int, C.c_float, C.c_int, C.c_float, vp, vp]
         L.vr_render_to_host.argtypes = [vp, cam, C.c_int, C.c_int, C.c_float, C.c_int, C.c_float, vp]
+        L.vr_render_to_host_async.argtypes = [vp, cam, C.c_int, C.c_int, C.c_float, C.c_int, C.c_float, vp]
+        L.vr_wait_frames.argtypes = [vp]
         L.vr_render_bricks.argtypes = [vp, cam, C.c_int, C.c_int, C.c_float, C.c_int, C.c_float, vp]
         L.vr_composite.argtypes = [vp, cam, C.c_int, C.c_int, C.c_int, vp, vp, vp]
         L.vr_plan_bricks.argtypes = [ip, ip, cam, C.c_int, C.c_int, vp, ip]
@@ -211,6 +213,16 @@ class Volume:
         _check(lib().vr_render_to_host(self._h, C.byref(cam), int(W), int(H), float(step), int(mode),
                                        float(ert_alpha), C.c_void_p(host_out.data_ptr())))
         return host_out
+
+    def vr_render_to_host_async(self, cam, W, H, step, mode, ert_alpha, host_out):
+        """As vr_render_to_host without the wait; host_out must stay untouched until vr_wait_frames()."""
+        assert not host_out.is_cuda and host_out.is_contiguous() and host_out.numel() == H * W * 4
+        _check(lib().vr_render_to_host_async(self._h, C.byref(cam), int(W), int(H), float(step), int(mode),
+                                             float(ert_alpha), C.c_void_p(host_out.data_ptr())))
+        return host_out
+
+    def vr_wait_frames(self):
+        _check(lib().vr_wait_frames(self._h))
 
     def vr_render_bricks(self, cam, W, H, step, mode, ert_alpha=0.0):
         import torch

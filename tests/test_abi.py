@@ -56,6 +56,8 @@ def test_null_and_range_checks_without_device(vr):
     cam = vr.camera_from_spec(wl.orbit_camera((8, 8, 8), 30, 20, wl.PROJ_ORTHO))
     assert L.vr_render(None, C.byref(cam), 8, 8, 1.0, 0, 0.0, None, None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_render_to_host(None, C.byref(cam), 8, 8, 1.0, 0, 0.0, None) == vr.VR_ERR_INVALID_ARG
+    assert L.vr_render_to_host_async(None, C.byref(cam), 8, 8, 1.0, 0, 0.0, None) == vr.VR_ERR_INVALID_ARG
+    assert L.vr_wait_frames(None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_measure(None, C.byref(cam), 8, 8, 1.0, 0, 0.0, None, None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_measure_units(None, C.byref(cam), 8, 8, 1.0, 0, 0.0, None, None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_set_empty_space_skipping(None, 1) == vr.VR_ERR_INVALID_ARG

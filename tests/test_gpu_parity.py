@@ -574,3 +574,27 @@ def test_channel_mask_matches_oracle(vr, oracle):
         vol.vr_set_channel_mask(many)
     assert err.value.status == vr.VR_ERR_INVALID_ARG
     vol.close()
+
+
+def test_render_to_host_async_delivers_the_same_frames(vr):
+    """vr_render_to_host_async + vr_wait_frames: frames of a short orbit delivered through the two alternating
+    device frames and the copy stream equal vr_render's, bit for bit, also when the image size changes."""
+    import torch
+    dims = (60, 50, 40)
+    cube = wl.cube_blobs(dims, 41, "cuda", n_blobs=5, amp=6.0, sigma=5.0)
+    vol = vr.Volume(cube)
+    vol.vr_set_transfer_function(wl.tf_ramp(0.2), -3.0, 8.0)
+    vol.vr_set_bricks(2, 2, 1)
+    for W, H in ((96, 80), (160, 120)):
+        cams = [vr.camera_from_spec(wl.orbit_camera(dims, az, 20.0, wl.PROJ_PERSP)) for az in (0.0, 50.0, 100.0, 150.0, 200.0)]
+        want = [vol.vr_render(c, W, H, 0.5, 0, 0.0).cpu() for c in cams]
+        bufs = [torch.empty((H, W, 4), dtype=torch.float32).pin_memory() for _ in cams]
+        for c, b in zip(cams, bufs):
+            vol.vr_render_to_host_async(c, W, H, 0.5, 0, 0.0, b)
+        vol.vr_wait_frames()
+        for a, b in zip(want, bufs):
+            assert torch.equal(a, b)
+        one = torch.empty((H, W, 4), dtype=torch.float32).pin_memory()
+        vol.vr_render_to_host(cams[2], W, H, 0.5, 0, 0.0, one)
+        assert torch.equal(one, want[2])
+    vol.close()
