@@ -54,6 +54,7 @@ struct FrameParams {
     int ert_on;
     int seg_len, seg_span;                    // samples per anchored segment; ceil(seg_len*step)+1 (sampler.cuh)
     int nbx, nby;                             // occupancy-mask words (4^3 cells) per row / per column
+    int pf_every, pf_ahead;                   // VR_EXP_L2PREFETCH builds only (env VR_PF), else 0
     int n_runs;                               // S2 channel mask: runs of enabled channels (0 = no mask)
     int run_z[2 * MAX_RUNS];                  // [za, zb) per run, ascending
 };
@@ -554,6 +555,9 @@ cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ 
         const unsigned slab_bytes = P.slab_stride * 4u;
         float vprev = 0.f;
         bool have = false, done = false;
+#ifdef VR_EXP_L2PREFETCH
+        unsigned pf_last = 0xffffffffu;
+#endif
         for (int js = 0; js < n && !done; js += P.seg_len) {
             // In the two-pass variants the ray is re-derived from the pixel here (same expressions, same doubles)
             // rather than kept: twelve live double registers across both passes spilled to local memory (measured:
@@ -601,6 +605,26 @@ cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ 
                 }
             } else {
                 for (int jl = 0; jl < je; ++jl) {
+#ifdef VR_EXP_L2PREFETCH
+                    // EXPERIMENT, rejected (profiles/r02_experiments.md).  Build: VR_DEFINES=-DVR_EXP_L2PREFETCH
+                    // python -m paper_1008_0135_b200.build; run with VR_PF=every,ahead.  Every `every` samples the ray
+                    // looks `ahead` samples on and, when that point lies in an 8^3 tile it has not asked for yet, has
+                    // the bulk-copy engine pull the whole 2 KB tile into the L2 (cp.async.bulk.prefetch.L2, SASS UBLKPF);
+                    // lanes that want the same tile are merged with match.any.
+                    if (P.pf_every && ((unsigned)(js + jl) & (unsigned)(P.pf_every - 1)) == 0u && js + jl + P.pf_ahead < n) {
+                        unsigned ax, ay, az;
+                        locate_cell(An, jl + P.pf_ahead, h, ax, ay, az);
+                        const unsigned tid = (az >> 3) * (P.slab_stride >> 9) + (ay >> 3) * (P.ty_stride >> 9) + (ax >> 3);
+                        if (tid != pf_last) {
+                            pf_last = tid;
+                            const unsigned peers = __match_any_sync(__activemask(), tid);
+                            if ((peers & ((1u << (threadIdx.x & 31)) - 1u)) == 0u) {
+                                const unsigned long long a = vol_base + (unsigned long long)tid * (TILE_ELEMS * 4ull);
+                                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(a), "r"(TILE_ELEMS * 4) : "memory");
+                            }
+                        }
+                    }
+#endif
                     Cell c;
                     locate(An, jl, h, c);
                     const float v = sample_cached(vol_base, P.ty_stride, slab_bytes, c, K);

@@ -69,6 +69,7 @@ struct vr_volume {
     // NEXT-2 empty-space skipping: occupancy mask (one bit per voxel cell), built for the current table on demand
     int n_runs = 0;                   // S2 channel mask as runs of enabled channels; 0 = every channel enabled
     int run_z[2 * vr::MAX_RUNS] = {0};
+    int pf_every = 0, pf_ahead = 0;   // experiment builds only (-DVR_EXP_L2PREFETCH): env VR_PF="every,ahead"
     int seg_max = 64;                 // samples (and voxels of path) per anchored segment; env VR_SEG overrides (1..64)
     bool skip_enabled = true;
     unsigned long long* d_mask = nullptr;
@@ -144,6 +145,7 @@ vr_status build_frame(const vr_volume* vol, const vr_camera* cam, int W, int H, 
     P.seg_len = std::max(1, std::min(vol->seg_max, (int)((double)vol->seg_max / (double)step)));
     P.seg_span = (int)std::ceil((double)P.seg_len * (double)step) + 1;
     P.nbx = vol->NBX; P.nby = vol->NBY;
+    P.pf_every = vol->pf_every; P.pf_ahead = vol->pf_ahead;
     P.n_runs = vol->n_runs;
     for (int k = 0; k < 2 * vr::MAX_RUNS; ++k) P.run_z[k] = vol->run_z[k];
     P.x_zero_below = table_zero_below(vol);   // the per-step opacity correction keeps zeros zero
@@ -310,6 +312,12 @@ vr_status vr_create_volume(const int dims[3], const float* d_data, vr_volume** o
     vr_volume* v = new (std::nothrow) vr_volume();
     if (!v) return fail(VR_ERR_OOM, "vr_create_volume: host allocation failed");
     for (int a = 0; a < 3; ++a) { v->dims[a] = dims[a]; v->sub_hi[a] = dims[a]; }
+    if (const char* pf = std::getenv("VR_PF")) {
+        int ev_ = 0, ah = 0;
+        if (std::sscanf(pf, "%d,%d", &ev_, &ah) == 2 && ev_ >= 0 && ev_ <= 64 && (ev_ & (ev_ - 1)) == 0 && ah >= 0 && ah <= 64) {
+            v->pf_every = ev_; v->pf_ahead = ah;
+        }
+    }
     if (const char* e_ = std::getenv("VR_SEG")) {          // tuning knob for measurements
         const int sv = std::atoi(e_);
         if (sv >= 1 && sv <= 64) v->seg_max = sv;
