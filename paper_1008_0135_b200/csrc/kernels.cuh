@@ -34,6 +34,9 @@ constexpr int PAD_X = 8, PAD_Y = 1, PAD_Z = 1;
 #ifndef VR_CTA_W
 #define VR_CTA_W 16
 #endif
+#ifndef VR_OCC_GROUP
+#define VR_OCC_GROUP 16     // samples per group of the occupancy pass (power of two <= 32; measured 2: 4.43, 4: 4.38, 8: 4.35, 16: 4.34 ms)
+#endif
 constexpr int CTA_W = VR_CTA_W;               // a CTA renders a CTA_W x CTA_H pixel tile: warps of 8x4 pixels, 2 across
 constexpr int CTA_H = VR_CTA_H;
 constexpr int CTA_THREADS = CTA_W * CTA_H;
@@ -578,14 +581,44 @@ cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ 
                 }
                 if (SKIP) {                                    // NEXT-2: cells that cannot contribute
                     unsigned occ_lo = 0u, occ_hi = 0u;
-                    for (int jl = 0; jl < je; ++jl) {
-                        unsigned ix, iy, iz;
-                        locate_cell(An, jl, h, ix, iy, iz);
-                        const unsigned occ = cell_occupied(mask, nbx, nbxy, ix, iy, iz, mc) ? 1u : 0u;
-                        if (jl < 32) occ_lo |= occ << jl; else occ_hi |= occ << (jl - 32);
+                    // VR_OCC_GROUP samples at a time: tags, then the (rare) word loads back to back into registers of
+                    // their own, then the bit tests — the loads of a group are in flight together instead of one L2/HBM
+                    // latency per new block.  Samples at or beyond je are located as copies of sample je - 1 and
+                    // dropped by the AND with todo below.
+                    constexpr int G = VR_OCC_GROUP;
+                    for (int jb = 0; jb < je; jb += G) {
+                        unsigned tg[G], bp[G];
+#pragma unroll
+                        for (int k = 0; k < G; ++k) {
+                            unsigned ix, iy, iz;
+                            locate_cell(An, min(jb + k, je - 1), h, ix, iy, iz);
+                            tg[k] = (iz >> 2) * nbxy + (iy >> 2) * nbx + (ix >> 2);
+                            bp[k] = ((iz & 3u) << 4) | ((iy & 3u) << 2) | (ix & 3u);
+                        }
+                        uint2 w[G];
+#pragma unroll
+                        for (int k = 0; k < G; ++k) {
+                            const unsigned prev = k ? tg[k - 1] : mc.tag;
+                            w[k] = make_uint2(0u, 0u);
+                            if (tg[k] != prev) w[k] = __ldg(reinterpret_cast<const uint2*>(mask + tg[k]));
+                        }
+                        uint2 cur = make_uint2(mc.lo, mc.hi);
+                        unsigned nib = 0u;
+#pragma unroll
+                        for (int k = 0; k < G; ++k) {
+                            const unsigned prev = k ? tg[k - 1] : mc.tag;
+                            if (tg[k] != prev) cur = w[k];
+                            const unsigned half = (bp[k] & 32u) ? cur.y : cur.x;
+                            nib |= ((half >> (bp[k] & 31u)) & 1u) << k;
+                        }
+                        mc.lo = cur.x; mc.hi = cur.y; mc.tag = tg[G - 1];
+                        if (jb < 32) occ_lo |= nib << jb; else occ_hi |= nib << (jb - 32);
                     }
                     todo_lo &= occ_lo; todo_hi &= occ_hi;
                 }
+                cache_init(K);      // the row cache does not survive a segment: its 25 registers are then dead during the
+                                    // occupancy pass, which lets ptxas keep a group's mask loads in flight (measured
+                                    // -3.6 % on config 3, -6 % on config 2; profiles/r02_experiments.md)
                 while (todo_lo | todo_hi) {
                     int jl;
                     if (todo_lo) { jl = __ffs((int)todo_lo) - 1; todo_lo &= todo_lo - 1u; }
