@@ -346,7 +346,8 @@ __device__ __forceinline__ void classify_blend(const float4* __restrict__ tf, co
 //     x_zero_below and both entries the lookup blends have alpha = 0 (O6) -> C and A unchanged (O7).
 // A clear bit therefore never changes a pixel: the oracle needs no rule for it, and parity gates stay as they are.
 // Layout: 64-bit words of 4x4x4 cells, word ((bz*NBY + by)*NBX + bx), bit (lz*4 + ly)*4 + lx.
-// One CTA = 32 x 8 x 8 cells (8 x 2 x 2 words): the 33 x 9 x 9 corner classes go through shared memory.
+// One CTA = 32 x 8 x 8 cells (8 x 2 x 2 words): each warp classifies rows of 33 corner voxels into two bit sets
+// (ballot), a cell row of 32 cells is then four ORs, a shift and an AND-NOT on 64-bit words.
 // ------------------------------------------------------------------------------------------------
 constexpr float MASK_MARGIN = 0.01f;       // in table entries (x units): far above fp32 rounding of the blend
 
@@ -354,39 +355,68 @@ __global__ void __launch_bounds__(256)
 build_mask_kernel(const float* __restrict__ vol, unsigned ty_stride, unsigned slab_stride, int nx, int ny, int nz,
                   float vmin, float inv_range, float x_zero_below, unsigned long long* __restrict__ mask, int NBX,
                   int NBY, unsigned long long* __restrict__ n_occupied) {
-    __shared__ unsigned char cls[9][9][36];    // 1 = may be visible, 2 = NaN
-    __shared__ unsigned words[2][2][8][2];     // [wz][wy][wx][half]
+    // per (z,y) row of the 33 x 9 x 9 corner voxels: bit x set when the voxel may be visible / is NaN
+    __shared__ unsigned long long vis[9][9], nanb[9][9];
+    __shared__ unsigned rowbits[8][8];          // [lz][ly]: the 32 cell bits of one cell row
     const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 8, z0 = blockIdx.z * 8;
     const int t = threadIdx.x;
-    if (t < 64) (&words[0][0][0][0])[t] = 0u;
-    for (int i = t; i < 9 * 9 * 33; i += 256) {
-        const int lx = i % 33, r = i / 33, ly = r % 9, lz = r / 9;
-        const int x = min(x0 + lx, nx + PAD_X), y = min(y0 + ly, ny + PAD_Y), z = min(z0 + lz, nz + PAD_Z);   // padded coordinates
-        const float v = __ldg(vol + tiled_index(x, y, z, ty_stride, slab_stride));
-        const float xt = __saturatef((v - vmin) * inv_range) * 255.0f;
-        cls[lz][ly][lx] = (v != v) ? 2 : (xt < x_zero_below - MASK_MARGIN ? 0 : 1);
-    }
+    const int x_last = (int)(ty_stride >> 9) * 8 - 1;            // last padded x that exists (TX * 8 - 1)
+    const float thr = x_zero_below - MASK_MARGIN;
+    if (t < 81) { (&vis[0][0])[t] = 0ull; (&nanb[0][0])[t] = 0ull; }
     __syncthreads();
-    const int lz = t >> 5, ly = (t >> 2) & 7, lxq = (t & 3) * 8;
-    unsigned bits = 0;
+    // 81 rows x (8 aligned 16-byte chunks + the 33rd voxel) = 729 items, three per thread: all loads first
+    float4 q[3];
 #pragma unroll
-    for (int k = 0; k < 8; ++k) {
-        const int lx = lxq + k;
-        const unsigned o = cls[lz][ly][lx] | cls[lz][ly][lx + 1] | cls[lz][ly + 1][lx] | cls[lz][ly + 1][lx + 1] |
-                           cls[lz + 1][ly][lx] | cls[lz + 1][ly][lx + 1] | cls[lz + 1][ly + 1][lx] | cls[lz + 1][ly + 1][lx + 1];
-        const bool in = (x0 + lx < nx + PAD_X) && (y0 + ly < ny + PAD_Y) && (z0 + lz < nz + PAD_Z);   // n_a + PAD_a padded cells per axis
-        if (in && (o & 1u) && !(o & 2u)) bits |= 1u << k;
+    for (int k = 0; k < 3; ++k) {
+        const int i = t + 256 * k;
+        q[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (i < 729) {
+            const int row = i / 9, ch = i - row * 9;
+            const int y = min(y0 + row % 9, ny + PAD_Y), z = min(z0 + row / 9, nz + PAD_Z);
+            if (ch < 8) q[k] = __ldg(reinterpret_cast<const float4*>(vol + tiled_index(min(x0 + 4 * ch, x_last - 3), y, z, ty_stride, slab_stride)));
+            else q[k].x = __ldg(vol + tiled_index(min(x0 + 32, x_last), y, z, ty_stride, slab_stride));
+        }
     }
-    // bits 0..3 -> word wx = 2*(t&3), bits 4..7 -> word wx + 1; bit position in the word: (lz&3)*16 + (ly&3)*4 + lx&3
-    const int wz = lz >> 2, wy = ly >> 2, pos = ((lz & 3) << 4) | ((ly & 3) << 2);
-    const unsigned lo4 = bits & 15u, hi4 = bits >> 4;
-    if (lo4) atomicOr(&words[wz][wy][2 * (t & 3)][pos >> 5], lo4 << (pos & 31));
-    if (hi4) atomicOr(&words[wz][wy][2 * (t & 3) + 1][pos >> 5], hi4 << (pos & 31));
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const int i = t + 256 * k;
+        if (i < 729) {
+            const int row = i / 9, ch = i - row * 9;
+            const float v[4] = {q[k].x, q[k].y, q[k].z, q[k].w};
+            unsigned long long bv = 0ull, bn = 0ull;
+            const int nv = ch < 8 ? 4 : 1;
+            for (int e = 0; e < nv; ++e) {
+                const float xt = __saturatef((v[e] - vmin) * inv_range) * 255.0f;
+                if (v[e] != v[e]) bn |= 1ull << e;
+                else if (!(xt < thr)) bv |= 1ull << e;
+            }
+            if (bv) atomicOr(&vis[row / 9][row % 9], bv << (4 * ch));
+            if (bn) atomicOr(&nanb[row / 9][row % 9], bn << (4 * ch));
+        }
+    }
     __syncthreads();
-    if (t < 32) {
+    if (t < 64) {                                                // one thread per cell row: 32 cells bit-parallel
+        const int ly = t & 7, lz = t >> 3;
+        const unsigned long long V = vis[lz][ly] | vis[lz][ly + 1] | vis[lz + 1][ly] | vis[lz + 1][ly + 1];
+        const unsigned long long N = nanb[lz][ly] | nanb[lz][ly + 1] | nanb[lz + 1][ly] | nanb[lz + 1][ly + 1];
+        unsigned occ = (unsigned)(V | (V >> 1)) & ~(unsigned)(N | (N >> 1));      // any corner visible, no corner NaN
+        const int n_in = nx + PAD_X - x0;                         // cells x0 + lx < nx + PAD_X exist
+        if (n_in < 32) occ &= n_in > 0 ? ((1u << n_in) - 1u) : 0u;
+        if (y0 + ly >= ny + PAD_Y || z0 + lz >= nz + PAD_Z) occ = 0u;
+        rowbits[lz][ly] = occ;
+    }
+    __syncthreads();
+    if (t < 32) {                                                // one thread per 64-bit word of 4x4x4 cells
         const int wx = t & 7, wyy = (t >> 3) & 1, wzz = t >> 4;
+        unsigned long long w = 0ull;
+#pragma unroll
+        for (int lz4 = 0; lz4 < 4; ++lz4)
+#pragma unroll
+            for (int ly4 = 0; ly4 < 4; ++ly4) {
+                const unsigned long long nib = (rowbits[wzz * 4 + lz4][wyy * 4 + ly4] >> (4 * wx)) & 15u;
+                w |= nib << ((lz4 * 4 + ly4) * 4);
+            }
         const int bx = blockIdx.x * 8 + wx, by = blockIdx.y * 2 + wyy, bz = blockIdx.z * 2 + wzz;
-        const unsigned long long w = (unsigned long long)words[wzz][wyy][wx][0] | ((unsigned long long)words[wzz][wyy][wx][1] << 32);
         const bool in = bx < NBX && by < NBY && bz * 4 < nz + PAD_Z;
         if (in) mask[((size_t)bz * NBY + by) * NBX + bx] = w;
         unsigned long long cnt = in ? (unsigned long long)__popcll(w) : 0ull;
