@@ -264,6 +264,34 @@ __device__ __forceinline__ long long lattice_index(double t, double t_near, doub
     return x > 0.0 ? (long long)x : 0ll;
 }
 
+// O3 + O4 + O9 for one (ray, brick): global clip, t_near, and the range [i_lo, i_lo + n) of the global lattice the
+// brick owns.  Returns n (0: miss or nothing owned).
+__device__ __forceinline__ int owned_samples(const FrameParams& P, const BrickRec* __restrict__ br, const double o[3],
+                                             const double d[3], double& t_near, long long& i_lo) {
+    const double glo[3] = {0.0, 0.0, 0.0};
+    const double ghi[3] = {(double)P.nx, (double)P.ny, (double)P.nz};
+    double tn, tf_;
+    bool hit = slab_clip(o, d, glo, ghi, tn, tf_);
+    if (tn < 0.0) tn = 0.0;
+    hit = hit && (tf_ > tn);
+    long long i_hi = 0;
+    i_lo = 0; t_near = 0.0;
+    if (hit) {
+        t_near = tn;
+        const double blo[3] = {(double)br->lo[0], (double)br->lo[1], (double)br->lo[2]};
+        const double bhi[3] = {(double)br->hi[0], (double)br->hi[1], (double)br->hi[2]};
+        double t0, t1;
+        bool bh = slab_clip(o, d, blo, bhi, t0, t1);
+        if (t0 < tn) t0 = tn;
+        if (t1 > tf_) t1 = tf_;
+        if (bh && t1 > t0) {
+            i_lo = lattice_index(t0, tn, P.step);
+            i_hi = lattice_index(t1, tn, P.step);
+        }
+    }
+    return (i_hi > i_lo) ? (int)(i_hi - i_lo) : 0;
+}
+
 // ------------------------------------------------------------------------------------------------
 // O5  plain 8-corner trilinear sample of one cell (measuring build only: marks the 32-byte sectors it reads).
 // ------------------------------------------------------------------------------------------------
@@ -502,30 +530,9 @@ cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ 
     // ---- per-ray set-up, double precision (O2-O4, O9) ----
     double o[3], d[3];
     make_ray(P, px, py, o, d);
-    long long i_lo = 0, i_hi = 0;
+    long long i_lo = 0;
     double t_near = 0.0;
-    {
-        const double glo[3] = {0.0, 0.0, 0.0};
-        const double ghi[3] = {(double)P.nx, (double)P.ny, (double)P.nz};
-        double tn, tf_;
-        bool hit = slab_clip(o, d, glo, ghi, tn, tf_);
-        if (tn < 0.0) tn = 0.0;
-        hit = hit && (tf_ > tn);
-        if (hit) {
-            t_near = tn;
-            const double blo[3] = {(double)br->lo[0], (double)br->lo[1], (double)br->lo[2]};
-            const double bhi[3] = {(double)br->hi[0], (double)br->hi[1], (double)br->hi[2]};
-            double t0, t1;
-            bool bh = slab_clip(o, d, blo, bhi, t0, t1);
-            if (t0 < tn) t0 = tn;
-            if (t1 > tf_) t1 = tf_;
-            if (bh && t1 > t0) {
-                i_lo = lattice_index(t0, tn, P.step);
-                i_hi = lattice_index(t1, tn, P.step);
-            }
-        }
-    }
-    const int n = (i_hi > i_lo) ? (int)(i_hi - i_lo) : 0;
+    const int n = owned_samples(P, br, o, d, t_near, i_lo);
 
     const size_t pix = (size_t)br->img_base + (size_t)(py - br->oy) * br->img_stride + (size_t)(px - br->ox);
     if (n == 0) {

@@ -1,0 +1,225 @@
+// slab.cuh — the slab-staged caster (north_star kernel (2): "brick slabs staged through shared memory via TMA
+// where the view is near axis-aligned"; section 2.4).
+//
+// When the rays of a frame are parallel (orthographic) and the pixel pitch times the step is small, many samples
+// fall into every voxel cell and the caster is bound by instruction issue, not by HBM (the ridge at
+// ~14 B per sample).  The row-cache sampler of sampler.cuh spends ~140 of its ~220 instructions per sample on
+// address formation, slot bookkeeping and selects.  Here a CTA instead marches its 16x8-pixel tile through the brick
+// SLAB BY SLAB along the rays' dominant axis: a slab is D cell layers thick; the box of voxels all its rays can touch
+// inside the slab (window, D + 1 layers with the far neighbours) is copied by ONE bulk tensor copy
+// (cp.async.bulk.tensor.3d, SASS UTMALDG) from a LINEAR padded copy of the cube into shared memory, double-buffered
+// with mbarriers, and the eight corners of a sample are eight LDS from one base address plus three adds.
+// Positions, cells and fractions come from the same segment-anchored arithmetic as the row-cache caster
+// (sampler.cuh: set_anchor / locate), the lattice, ownership and termination rules are unchanged (O4, O7, O9).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace vr {
+
+// Linear padded copy: float lin[LZ][LY][LX] in the PADDED coordinates of the tiled copy (u = voxel + PAD), so the
+// replicated layers are O5's clamp-to-edge here too.  LX is a multiple of 4 (row pitch a multiple of 16 B for TMA).
+struct LinearDims {
+    int LX, LY, LZ;
+};
+__host__ __device__ inline LinearDims linear_dims(int nx, int ny, int nz) {
+    LinearDims L;
+    L.LX = (nx + PAD_X + 1 + 3) & ~3;
+    L.LY = ny + PAD_Y + 1;
+    L.LZ = nz + PAD_Z + 1;
+    return L;
+}
+
+// tiled copy -> linear padded copy: one thread per 16-byte chunk (4 voxels along x); reads whole 32-byte tile rows
+// per pair of lanes, writes 512 contiguous bytes per warp.
+__global__ void __launch_bounds__(256)
+linearize_kernel(const float* __restrict__ tiled, float* __restrict__ lin, int LX, int LY, int LZ, unsigned ty_stride,
+                 unsigned slab_stride) {
+    const int cx = blockIdx.x * 64 + (threadIdx.x & 63);        // chunk index along x
+    const int y = blockIdx.y * 4 + (threadIdx.x >> 6);
+    const int z = blockIdx.z;
+    if (cx * 4 >= LX || y >= LY) return;
+    const float4 v = __ldcs(reinterpret_cast<const float4*>(tiled + tiled_index(cx * 4, y, z, ty_stride, slab_stride)));
+    *reinterpret_cast<float4*>(lin + ((size_t)z * LY + y) * LX + cx * 4) = v;
+}
+
+struct SlabParams {
+    int logD;                 // slab thickness D = 1 << logD cell layers along the dominant axis
+    int w[3];                 // window extent in voxels per axis (dominant axis: D + 1; x: + 3 for the aligned start, a multiple of 4)
+    int box_floats;           // w[0]*w[1]*w[2]: what one bulk tensor copy delivers
+    int slot_floats;          // floats per buffer: box_floats rounded up to a multiple of 32 (buffers stay 128-byte aligned)
+    // orthographic rays of a CTA tile: padded position of the ray of pixel (px,py) where its dominant coordinate is c:
+    //   U_a(c) = base_a + px * dpx_a + py * dpy_a + c * slope_a   (a = the two other axes; slope = d_a / d_dom)
+    double base[3], dpx[3], dpy[3], slope[3];
+};
+
+// ---- mbarrier / TMA primitives (PTX ISA: mbarrier, cp.async.bulk.tensor) ----
+__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_addr(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, unsigned long long* bar, int c0, int c1, int c2) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+        ::"r"(smem_addr(dst)), "l"(reinterpret_cast<unsigned long long>(map)), "r"(smem_addr(bar)), "r"(c0), "r"(c1), "r"(c2)
+        : "memory");
+}
+
+
+// ------------------------------------------------------------------------------------------------
+// a1 + a3 + a4/a5, slab-staged.  Same grid and CTA shape as cast_kernel (16x8-pixel tiles per brick rectangle).
+// DOM = the rays' dominant axis.  Dynamic shared memory: [2 window buffers][256 float4 table][2 mbarriers][origins].
+// ------------------------------------------------------------------------------------------------
+template <int MODE, int DOM>
+__global__ void __launch_bounds__(CTA_THREADS)
+cast_slab_kernel(const __grid_constant__ FrameParams P, const __grid_constant__ SlabParams S,
+                 const __grid_constant__ CUtensorMap tmap, const BrickRec* __restrict__ bricks, int n_bricks,
+                 const float4* __restrict__ tf_global, float* __restrict__ img) {
+    extern __shared__ unsigned char smem_raw[];
+    // carve: windows first (128-byte aligned for the bulk tensor copy)
+    unsigned char* sb = smem_raw + ((128u - (smem_addr(smem_raw) & 127u)) & 127u);
+    float* win = reinterpret_cast<float*>(sb);
+    float4* tf = reinterpret_cast<float4*>(sb + (size_t)2 * S.slot_floats * 4);
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(tf + 256);
+    int* s_org = reinterpret_cast<int*>(bar + 2);          // [2][4]: window origin per buffer
+    int* s_misc = s_org + 8;                               // [0] brick, [1] min slab, [2] max slab
+
+    const int tid = threadIdx.x;
+    if (MODE == MODE_EA)
+        for (int i = tid; i < 256; i += CTA_THREADS) tf[i] = tf_global[i];
+    if (tid == 0) {
+        int lo = 0, hi = n_bricks - 1;
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (bricks[mid].tile0 <= (int)blockIdx.x) lo = mid; else hi = mid - 1;
+        }
+        s_misc[0] = lo; s_misc[1] = 0x7fffffff; s_misc[2] = -0x7fffffff;
+        mbar_init(&bar[0], 1); mbar_init(&bar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const BrickRec* __restrict__ br = bricks + s_misc[0];
+    const int tloc = (int)blockIdx.x - br->tile0;
+    const int tiles_x = br->tiles_x;
+    const int tyi = tloc / tiles_x, txi = tloc - tyi * tiles_x;
+    const int warp = tid >> 5, lane = tid & 31;
+    constexpr int WW = VR_WARP_W, WH = 32 / VR_WARP_W, WPR = CTA_W / WW;
+    const int lx = txi * CTA_W + (warp % WPR) * WW + (lane % WW);
+    const int ly = tyi * CTA_H + (warp / WPR) * WH + (lane / WW);
+    const bool inside = lx < br->rw && ly < br->rh;
+    const int px = br->rx0 + lx, py = br->ry0 + ly;
+
+    double o[3], d[3];
+    make_ray(P, px, py, o, d);
+    long long i_lo = 0;
+    double t_near = 0.0;
+    const int n = inside ? owned_samples(P, br, o, d, t_near, i_lo) : 0;
+    const float h[3] = {(float)(P.step * d[0]), (float)(P.step * d[1]), (float)(P.step * d[2])};
+    const int logD = S.logD;
+
+    Anchor An;
+    int js = 0;                                            // first sample of the current segment
+    if (n > 0) {                                           // slab range of this ray: its first and its last sample
+        Cell c;
+        set_anchor(o, d, t_near, P.step, i_lo + (n - 1), h, P.seg_span, An);
+        locate(An, 0, h, c);
+        const int c_last = (int)(DOM == 0 ? c.ix : DOM == 1 ? c.iy : c.iz) >> logD;
+        set_anchor(o, d, t_near, P.step, i_lo, h, P.seg_span, An);
+        locate(An, 0, h, c);
+        const int c_first = (int)(DOM == 0 ? c.ix : DOM == 1 ? c.iy : c.iz) >> logD;
+        atomicMin(&s_misc[1], min(c_first, c_last));
+        atomicMax(&s_misc[2], max(c_first, c_last));
+    }
+    __syncthreads();
+    const int s_min = s_misc[1], s_max = s_misc[2];
+    const int ns = s_max >= s_min ? s_max - s_min + 1 : 0;
+    const int sgn = P.fwd[DOM] >= 0.0 ? 1 : -1;            // orthographic: every ray has direction fwd
+    const int s_begin = sgn > 0 ? s_min : s_max;
+
+    // window origin of a slab on the two other axes: min over the tile's corner rays at both faces of the slab
+    constexpr int A1 = (DOM + 1) % 3, A2 = (DOM + 2) % 3;
+    double lo1 = 0.0, lo2 = 0.0;
+    if (tid == 0) {
+        const int px0 = br->rx0 + txi * CTA_W, py0 = br->ry0 + tyi * CTA_H;
+        lo1 = S.base[A1] + px0 * S.dpx[A1] + py0 * S.dpy[A1] + fmin(0.0, (CTA_W - 1) * S.dpx[A1]) + fmin(0.0, (CTA_H - 1) * S.dpy[A1]);
+        lo2 = S.base[A2] + px0 * S.dpx[A2] + py0 * S.dpy[A2] + fmin(0.0, (CTA_W - 1) * S.dpx[A2]) + fmin(0.0, (CTA_H - 1) * S.dpy[A2]);
+    }
+    const unsigned box_bytes = (unsigned)S.box_floats * 4u;
+    auto issue = [&](int k) {                              // thread 0: start the copy of slab k into buffer k & 1
+        const int s = s_begin + sgn * k, slot = k & 1;
+        const double c0 = (double)(s << logD), c1 = c0 + (double)(1 << logD);
+        int org[3];
+        org[DOM] = s << logD;
+        org[A1] = (int)floor(lo1 + fmin(c0 * S.slope[A1], c1 * S.slope[A1])) - 1;
+        org[A2] = (int)floor(lo2 + fmin(c0 * S.slope[A2], c1 * S.slope[A2])) - 1;
+        org[0] &= ~3;                                      // the copy must start 16-byte aligned (measured: a start
+                                                           // coordinate that is not a multiple of 4 floats faults)
+        s_org[slot * 4 + 0] = org[0]; s_org[slot * 4 + 1] = org[1]; s_org[slot * 4 + 2] = org[2];
+        mbar_expect_tx(&bar[slot], box_bytes);
+        tma_load_3d(win + (size_t)slot * S.slot_floats, &tmap, &bar[slot], org[0], org[1], org[2]);
+    };
+    if (tid == 0 && ns > 0) issue(0);
+
+    float Cr = 0.f, Cg = 0.f, Cb = 0.f, A = 0.f, M = -INFINITY;
+    int j = 0;
+    const int w0 = S.w[0], w01 = S.w[0] * S.w[1];
+    for (int k = 0; k < ns; ++k) {
+        const int slot = k & 1;
+        const int any = __syncthreads_or(j < n);           // every thread is done with slab k - 1 (buffer (k + 1) & 1)
+        if (any && tid == 0 && k + 1 < ns) issue(k + 1);
+        mbar_wait(&bar[slot], (unsigned)(k >> 1) & 1u);    // slab k has landed (it was issued in any case)
+        if (!any) break;
+        const int s = s_begin + sgn * k;
+        const float* __restrict__ wbase = win + (size_t)slot * S.slot_floats
+                                          - (s_org[slot * 4 + 0] + s_org[slot * 4 + 1] * w0 + s_org[slot * 4 + 2] * w01);
+        while (j < n) {
+            int jl = j - js;
+            if (jl == P.seg_len) {
+                js = j; jl = 0;
+                set_anchor(o, d, t_near, P.step, i_lo + js, h, P.seg_span, An);
+            }
+            Cell c;
+            locate(An, jl, h, c);
+            if (((int)(DOM == 0 ? c.ix : DOM == 1 ? c.iy : c.iz) >> logD) != s) break;
+            const float* __restrict__ p0 = wbase + ((int)c.ix + (int)c.iy * w0 + (int)c.iz * w01);
+            const float* __restrict__ p1 = p0 + w0;
+            const float* __restrict__ p2 = p0 + w01;
+            const float* __restrict__ p3 = p2 + w0;
+            const float c00 = fmaf(c.fx, p0[1] - p0[0], p0[0]);
+            const float c10 = fmaf(c.fx, p1[1] - p1[0], p1[0]);
+            const float c01 = fmaf(c.fx, p2[1] - p2[0], p2[0]);
+            const float c11 = fmaf(c.fx, p3[1] - p3[0], p3[0]);
+            const float c0 = fmaf(c.fy, c10 - c00, c00);
+            const float c1 = fmaf(c.fy, c11 - c01, c01);
+            const float v = fmaf(c.fz, c1 - c0, c0);
+            ++j;
+            if (MODE == MODE_EA) {
+                classify_blend(tf, P, v, Cr, Cg, Cb, A);
+                if (P.ert_on && A >= P.ert) j = n;
+            } else {
+                M = fmaxf(M, v);
+            }
+        }
+    }
+    if (!inside) return;
+    const size_t pix = (size_t)br->img_base + (size_t)(py - br->oy) * br->img_stride + (size_t)(px - br->ox);
+    if (MODE == MODE_EA) reinterpret_cast<float4*>(img)[pix] = make_float4(Cr, Cg, Cb, A);
+    else img[pix] = M;
+}
+
+}  // namespace vr

@@ -13,6 +13,7 @@
 
 #include "../../include/vr.h"
 #include "kernels.cuh"
+#include "slab.cuh"
 #include "plan.h"
 
 namespace {
@@ -80,6 +81,13 @@ struct vr_volume {
     float mask_key[3] = {0.f, 0.f, 0.f};   // vmin, inv_range, x_zero_below the mask was built for
     float mask_build_ms = 0.f;
     long long mask_occupied = 0;
+    // slab-staged caster (slab.cuh): linear padded copy, made on first use
+    int slab_mode = 1;                // 0 off, 1 auto (dense orthographic frames), 2 whenever the window fits
+    int slab_logd = -1;               // env VR_SLAB_LOGD: force the slab thickness (tuning), -1 = heuristic
+    float* d_linear = nullptr;
+    bool linear_failed = false;       // allocation failed once: stay on the row-cache caster
+    float linearize_ms = 0.f;
+    int last_slab[6] = {0, 0, 0, 0, 0, 0};   // last frame: used, dominant axis, D, window x, y, z
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};   // cast begin/end, composite begin/end
     bool timed_cast = false, timed_comp = false;
 };
@@ -271,6 +279,193 @@ vr_status launch_cast(vr_volume* vol, const Frame& f, int mode, float* d_img, un
     return VR_OK;
 }
 
+// ---- slab-staged caster (slab.cuh): eligibility, window sizing, tensor map, launch ----
+struct SlabPlan {
+    bool use = false;
+    int dom = 2;
+    vr::SlabParams S;
+    size_t smem = 0;
+    CUtensorMap map;
+};
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+constexpr size_t SLAB_SMEM_EXTRA = 4096 + 16 + 32 + 16 + 128;   // table, barriers, origins, misc, alignment slack
+
+// Decide whether this frame runs on the slab-staged caster and size its window.  Orthographic frames only: the rays
+// of a CTA tile are parallel, so the window has one size for every tile and slab.
+void plan_slab(const vr_volume* vol, const vr::FrameParams& P, int mode, bool skip_active, SlabPlan& sp) {
+    sp.use = false;
+    if (vol->slab_mode == 0 || P.proj != VR_PROJ_ORTHO || P.n_runs > 0 || vol->linear_failed) return;
+    if (skip_active && vol->slab_mode != 2) return;          // the skipping caster drops most samples of such frames
+    (void)mode;
+    int dom = 0;
+    for (int a = 1; a < 3; ++a) if (std::fabs(P.fwd[a]) > std::fabs(P.fwd[dom])) dom = a;
+    const double pad[3] = {(double)vr::PAD_X, (double)vr::PAD_Y, (double)vr::PAD_Z};
+    double q0[3], dqx[3], dqy[3];                            // padded position of the pixel's ray origin, affine in (px,py)
+    for (int a = 0; a < 3; ++a) {
+        q0[a] = P.eye[a] + (1.0 / P.W - 1.0) * P.h * P.asp * P.right[a] + (1.0 / P.H - 1.0) * P.h * P.up[a] + pad[a] - 0.5;
+        dqx[a] = 2.0 * P.h * P.asp * P.right[a] / P.W;
+        dqy[a] = 2.0 * P.h * P.up[a] / P.H;
+    }
+    vr::SlabParams& S = sp.S;
+    for (int a = 0; a < 3; ++a) {
+        S.slope[a] = P.fwd[a] / P.fwd[dom];
+        S.base[a] = q0[a] - q0[dom] * S.slope[a];
+        S.dpx[a] = dqx[a] - dqx[dom] * S.slope[a];
+        S.dpy[a] = dqy[a] - dqy[dom] * S.slope[a];
+    }
+    int best = -1;
+    for (int pass = 0; pass < 2 && best < 0; ++pass) {
+        const size_t budget = pass == 0 ? (size_t)56 * 1024 : (size_t)113 * 1024;   // 4 or 2 CTAs per SM
+        for (int logd = 3; logd >= 0; --logd) {
+            if (vol->slab_logd >= 0 && logd != vol->slab_logd) continue;
+            const int D = 1 << logd;
+            long long fl = 1;
+            bool fits = true;
+            for (int a = 0; a < 3; ++a) {
+                int w;
+                if (a == dom) w = D + 1;
+                else w = (int)std::ceil((vr::CTA_W - 1) * std::fabs(S.dpx[a]) + (vr::CTA_H - 1) * std::fabs(S.dpy[a]) +
+                                        D * std::fabs(S.slope[a])) + 5;
+                if (a == 0) w = (w + 3 + 3) & ~3;          // + 3: the copy starts at a multiple of 4 voxels
+                if (w > 256) fits = false;
+                fl *= w;
+            }
+            const size_t smem = (size_t)2 * (size_t)((fl + 31) & ~31ll) * 4 + SLAB_SMEM_EXTRA;
+            if (fits && smem <= budget) { best = logd; break; }
+        }
+    }
+    if (best < 0) return;
+    const int D = 1 << best;
+    S.logD = best;
+    long long fl = 1;
+    for (int a = 0; a < 3; ++a) {
+        int w;
+        if (a == dom) w = D + 1;
+        else w = (int)std::ceil((vr::CTA_W - 1) * std::fabs(S.dpx[a]) + (vr::CTA_H - 1) * std::fabs(S.dpy[a]) +
+                                D * std::fabs(S.slope[a])) + 5;
+        if (a == 0) w = (w + 3 + 3) & ~3;          // + 3: the copy starts at a multiple of 4 voxels
+        S.w[a] = w;
+        fl *= w;
+    }
+    S.box_floats = (int)fl;
+    S.slot_floats = (int)((fl + 31) & ~31ll);
+    sp.smem = (size_t)2 * S.slot_floats * 4 + SLAB_SMEM_EXTRA;
+    sp.dom = dom;
+    if (vol->slab_mode == 1) {
+        // auto: only where the frame is on the instruction-bound side of the ridge: window bytes per
+        // sample of a CTA tile below ~16 B (a ray takes D / (|fwd_dom| step) samples per slab)
+        const double samples = (double)vr::CTA_THREADS * D / (std::fabs(P.fwd[dom]) * P.step);
+        if ((double)S.box_floats * 4.0 / samples > 16.0) return;
+    }
+    sp.use = true;
+}
+
+vr_status ensure_linear(vr_volume* vol) {
+    if (vol->d_linear) return VR_OK;
+    const vr::LinearDims L = vr::linear_dims(vol->dims[0], vol->dims[1], vol->dims[2]);
+    cudaError_t e = cudaMalloc(&vol->d_linear, (size_t)L.LX * L.LY * L.LZ * sizeof(float));
+    if (e != cudaSuccess) { vol->d_linear = nullptr; vol->linear_failed = true; cudaGetLastError(); return cuda_fail(e, "allocate linear copy"); }
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    e = cudaEventCreate(&e0);
+    if (e == cudaSuccess) e = cudaEventCreate(&e1);
+    if (e == cudaSuccess) e = cudaEventRecord(e0, vol->stream);
+    if (e == cudaSuccess) {
+        dim3 grid((L.LX / 4 + 63) / 64, (L.LY + 3) / 4, L.LZ);
+        vr::linearize_kernel<<<grid, 256, 0, vol->stream>>>(vol->d_tiled, vol->d_linear, L.LX, L.LY, L.LZ,
+                                                            (unsigned)vol->TX * vr::TILE_ELEMS,
+                                                            (unsigned)vol->TX * (unsigned)vol->TY * vr::TILE_ELEMS);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaEventRecord(e1, vol->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(vol->stream);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&vol->linearize_ms, e0, e1);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (e != cudaSuccess) { cudaFree(vol->d_linear); vol->d_linear = nullptr; vol->linear_failed = true; return cuda_fail(e, "linearize"); }
+    return VR_OK;
+}
+
+vr_status encode_slab_map(vr_volume* vol, SlabPlan& sp) {
+    EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc) return fail(VR_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
+    const vr::LinearDims L = vr::linear_dims(vol->dims[0], vol->dims[1], vol->dims[2]);
+    const cuuint64_t gdim[3] = {(cuuint64_t)L.LX, (cuuint64_t)L.LY, (cuuint64_t)L.LZ};
+    const cuuint64_t gstr[2] = {(cuuint64_t)L.LX * 4, (cuuint64_t)L.LX * L.LY * 4};
+    const cuuint32_t box[3] = {(cuuint32_t)sp.S.w[0], (cuuint32_t)sp.S.w[1], (cuuint32_t)sp.S.w[2]};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    const CUresult r = enc(&sp.map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, vol->d_linear, gdim, gstr, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(VR_ERR_CUDA, "cuTensorMapEncodeTiled failed (code " + std::to_string((int)r) + ")");
+    return VR_OK;
+}
+
+template <int MODE, int DOM>
+vr_status launch_slab_t(vr_volume* vol, const Frame& f, const SlabPlan& sp, float* d_img) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        VR_CUDA(cudaFuncSetAttribute(vr::cast_slab_kernel<MODE, DOM>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024),
+                "cudaFuncSetAttribute(slab caster)");
+        attr_set = true;
+    }
+    vr::cast_slab_kernel<MODE, DOM><<<f.total_tiles, vr::CTA_THREADS, sp.smem, vol->stream>>>(
+        f.P, sp.S, sp.map, vol->d_bricks, (int)f.recs.size(), vol->d_tf_ea, d_img);
+    VR_CUDA(cudaGetLastError(), "slab caster launch");
+    return VR_OK;
+}
+
+vr_status launch_slab(vr_volume* vol, const Frame& f, const SlabPlan& sp, int mode, float* d_img) {
+    if (f.total_tiles == 0) return VR_OK;
+    if (mode == VR_MODE_EA) {
+        if (sp.dom == 0) return launch_slab_t<vr::MODE_EA, 0>(vol, f, sp, d_img);
+        if (sp.dom == 1) return launch_slab_t<vr::MODE_EA, 1>(vol, f, sp, d_img);
+        return launch_slab_t<vr::MODE_EA, 2>(vol, f, sp, d_img);
+    }
+    if (sp.dom == 0) return launch_slab_t<vr::MODE_MIP, 0>(vol, f, sp, d_img);
+    if (sp.dom == 1) return launch_slab_t<vr::MODE_MIP, 1>(vol, f, sp, d_img);
+    return launch_slab_t<vr::MODE_MIP, 2>(vol, f, sp, d_img);
+}
+
+// The product caster of one frame: the slab-staged kernel where plan_slab says so, else the row-cache kernel.
+vr_status cast_frame(vr_volume* vol, const Frame& f, int mode, float* d_img) {
+    const bool skip = skip_applies(vol, mode);
+    SlabPlan sp;
+    plan_slab(vol, f.P, mode, skip, sp);
+    if (sp.use && ensure_linear(vol) != VR_OK) sp.use = false;            // no memory for the second copy: row-cache caster
+    if (sp.use) {
+        vr_status s = encode_slab_map(vol, sp);
+        if (s != VR_OK) return s;
+    }
+    vol->last_slab[0] = sp.use ? 1 : 0;
+    if (sp.use) {
+        vol->last_slab[1] = sp.dom; vol->last_slab[2] = 1 << sp.S.logD;
+        for (int a = 0; a < 3; ++a) vol->last_slab[3 + a] = sp.S.w[a];
+        return launch_slab(vol, f, sp, mode, d_img);
+    }
+    if (skip) {
+        vr_status s = ensure_mask(vol);                                   // builds only after a table change
+        if (s != VR_OK) return s;
+    }
+    return launch_cast<0>(vol, f, mode, d_img, nullptr, nullptr, nullptr);
+}
+
 vr_status launch_composite(vr_volume* vol, const Frame& f, int mode, const float* d_img, int W, int H, float* d_out,
                            float* d_scalar) {
     const int B = (int)f.recs.size();
@@ -317,6 +512,10 @@ vr_status vr_create_volume(const int dims[3], const float* d_data, vr_volume** o
         if (std::sscanf(pf, "%d,%d", &ev_, &ah) == 2 && ev_ >= 0 && ev_ <= 64 && (ev_ & (ev_ - 1)) == 0 && ah >= 0 && ah <= 64) {
             v->pf_every = ev_; v->pf_ahead = ah;
         }
+    }
+    if (const char* e_ = std::getenv("VR_SLAB_LOGD")) {     // tuning knob: slab thickness 2^k cell layers
+        const int sv = std::atoi(e_);
+        if (sv >= 0 && sv <= 3) v->slab_logd = sv;
     }
     if (const char* e_ = std::getenv("VR_SEG")) {          // tuning knob for measurements
         const int sv = std::atoi(e_);
@@ -394,6 +593,7 @@ void vr_destroy_volume(vr_volume* v) {
     }
     if (v->copy_stream) cudaStreamDestroy(v->copy_stream);
     if (v->d_mask) cudaFree(v->d_mask);
+    if (v->d_linear) cudaFree(v->d_linear);
     if (v->d_mask_count) cudaFree(v->d_mask_count);
     for (int k = 0; k < 4; ++k)
         if (v->ev[k]) cudaEventDestroy(v->ev[k]);
@@ -482,9 +682,14 @@ vr_status vr_render(vr_volume* vol, const vr_camera* cam, int W, int H, float st
     vol->timed_cast = vol->timed_comp = false;
     if (!direct && (s = ensure_pool(vol, f.pool_pixels * (mode == VR_MODE_EA ? 4 : 1),
                                     (size_t)B * W * H * (mode == VR_MODE_EA ? 4 : 1))) != VR_OK) return s;
-    if (skip_applies(vol, mode) && (s = ensure_mask(vol)) != VR_OK) return s;   // builds only after a table change
+    {   // per-table / per-volume preparations stay outside the timed region of the frame
+        SlabPlan sp;
+        plan_slab(vol, f.P, mode, skip_applies(vol, mode), sp);
+        if (sp.use) ensure_linear(vol);
+        else if (skip_applies(vol, mode) && (s = ensure_mask(vol)) != VR_OK) return s;
+    }
     VR_CUDA(cudaEventRecord(vol->ev[0], vol->stream), "record event");
-    s = launch_cast<0>(vol, f, mode, direct ? d_out_rgba : vol->d_pool, nullptr, nullptr, nullptr);
+    s = cast_frame(vol, f, mode, direct ? d_out_rgba : vol->d_pool);
     if (s != VR_OK) return s;
     VR_CUDA(cudaEventRecord(vol->ev[1], vol->stream), "record event");
     vol->timed_cast = true;
@@ -572,8 +777,7 @@ vr_status vr_render_bricks(vr_volume* vol, const vr_camera* cam, int W, int H, f
     const size_t n = B * (size_t)W * H * (mode == VR_MODE_EA ? 4 : 1);
     vr::fill_kernel<<<1184, 256, 0, vol->stream>>>(d_brick_images, n, mode == VR_MODE_EA ? 0.0f : -INFINITY);
     VR_CUDA(cudaGetLastError(), "fill kernel launch");
-    if (skip_applies(vol, mode) && (s = ensure_mask(vol)) != VR_OK) return s;
-    return launch_cast<0>(vol, f, mode, d_brick_images, nullptr, nullptr, nullptr);
+    return cast_frame(vol, f, mode, d_brick_images);
 }
 
 vr_status vr_composite(vr_volume* vol, const vr_camera* cam, int W, int H, int mode, const float* d_brick_images,
@@ -678,6 +882,24 @@ vr_status vr_get_skip_info(vr_volume* vol, int* h_active, float* h_build_ms, lon
     if (h_mask_bytes) *h_mask_bytes = active ? (long long)(vol->mask_words * sizeof(unsigned long long)) : 0;
     if (h_occupied_fraction)
         *h_occupied_fraction = active ? (double)vol->mask_occupied / ((double)vol->dims[0] * vol->dims[1] * vol->dims[2]) : 1.0;
+    return VR_OK;
+}
+
+vr_status vr_set_slab_staging(vr_volume* vol, int mode) {
+    if (!vol) return fail(VR_ERR_INVALID_ARG, "vr_set_slab_staging: volume is NULL");
+    if (mode < 0 || mode > 2) return fail(VR_ERR_INVALID_ARG, "vr_set_slab_staging: mode must be 0 (off), 1 (auto) or 2 (whenever it fits)");
+    vol->slab_mode = mode;
+    return VR_OK;
+}
+
+vr_status vr_get_slab_info(const vr_volume* vol, int h_info[6], float* h_linearize_ms, long long* h_linear_bytes) {
+    if (!vol) return fail(VR_ERR_INVALID_ARG, "vr_get_slab_info: volume is NULL");
+    if (h_info) for (int k = 0; k < 6; ++k) h_info[k] = vol->last_slab[k];
+    if (h_linearize_ms) *h_linearize_ms = vol->linearize_ms;
+    if (h_linear_bytes) {
+        const vr::LinearDims L = vr::linear_dims(vol->dims[0], vol->dims[1], vol->dims[2]);
+        *h_linear_bytes = vol->d_linear ? (long long)L.LX * L.LY * L.LZ * 4 : 0;
+    }
     return VR_OK;
 }
 

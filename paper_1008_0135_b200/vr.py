@@ -21,7 +21,7 @@ VR_MAX_CHANNEL_RUNS = 16
 SYMBOLS = ["vr_create_volume", "vr_destroy_volume", "vr_set_stream", "vr_set_transfer_function",
            "vr_set_bricks", "vr_set_subcube", "vr_set_channel_mask", "vr_render", "vr_render_to_host", "vr_render_to_host_async", "vr_wait_frames", "vr_render_bricks", "vr_composite",
            "vr_plan_bricks", "vr_measure", "vr_measure_units", "vr_set_empty_space_skipping", "vr_get_skip_info",
-           "vr_set_l2_fetch_granularity",
+           "vr_set_l2_fetch_granularity", "vr_set_slab_staging", "vr_get_slab_info",
            "vr_get_l2_fetch_granularity", "vr_get_stage_ms", "vr_volume_info", "vr_volume_range", "vr_volume_histogram", "vr_export_linear", "vr_last_error"]
 
 
@@ -71,6 +71,8 @@ def lib():
         L.vr_set_empty_space_skipping.argtypes = [vp, C.c_int]
         L.vr_get_skip_info.argtypes = [vp, ip, fp, C.POINTER(C.c_longlong), C.POINTER(C.c_double)]
         L.vr_set_l2_fetch_granularity.argtypes = [C.c_int]
+        L.vr_set_slab_staging.argtypes = [vp, C.c_int]
+        L.vr_get_slab_info.argtypes = [vp, ip, fp, C.POINTER(C.c_longlong)]
         L.vr_get_l2_fetch_granularity.argtypes = [ip]
         L.vr_get_stage_ms.argtypes = [vp, fp, fp]
         L.vr_volume_info.argtypes = [vp, fp, C.POINTER(C.c_longlong)]
@@ -258,6 +260,17 @@ class Volume:
 
     def vr_set_empty_space_skipping(self, enabled):
         _check(lib().vr_set_empty_space_skipping(self._h, 1 if enabled else 0))
+
+    def vr_set_slab_staging(self, mode):
+        _check(lib().vr_set_slab_staging(self._h, int(mode)))
+
+    def vr_get_slab_info(self):
+        info = (C.c_int * 6)()
+        ms = C.c_float(0.0)
+        nb = C.c_longlong(0)
+        _check(lib().vr_get_slab_info(self._h, info, C.byref(ms), C.byref(nb)))
+        return {"used": bool(info[0]), "dominant_axis": info[1], "slab_layers": info[2],
+                "window": (info[3], info[4], info[5]), "linearize_ms": ms.value, "linear_bytes": nb.value}
 
     def vr_get_skip_info(self):
         """dict(active, build_ms, mask_bytes, occupied_fraction); builds the mask if it is due."""
