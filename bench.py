@@ -223,6 +223,8 @@ def run_ours(args):
     vol.vr_set_transfer_function(w.table, w.vmin, w.vmax)
     vol.vr_set_bricks(*w.bricks)
     vol.vr_set_empty_space_skipping(not args.no_skip)
+    if args.slab is not None:
+        vol.vr_set_slab_staging(args.slab)
     skip_info = vol.vr_get_skip_info()                           # builds the occupancy mask once (a per-table step)
     B = w.bricks[0] * w.bricks[1] * w.bricks[2]
     cams = [vr.camera_from_spec(w.camera(az_deg=a)) for a in views]
@@ -462,6 +464,8 @@ def run_sweep(args):
     vol = vr.Volume(cube)
     vol.vr_set_transfer_function(w.table, w.vmin, w.vmax)
     vol.vr_set_empty_space_skipping(not args.no_skip)
+    if args.slab is not None:
+        vol.vr_set_slab_staging(args.slab)
     cs = wl.orbit_camera(w.dims, 30.0, 20.0, wl.PROJ_ORTHO)
     cam = vr.camera_from_spec(cs)
     peak, peak_src = measured_peak_gbs()
@@ -509,7 +513,7 @@ def run_sweep(args):
                           "hbm_GBps_algorithmic": 32e-9 * sectors / (cast_med * 1e-3),
                           "frac_of_peak": 32e-9 * sectors / (cast_med * 1e-3) / peak, "peak": peak,
                           "side_of_ridge": "hbm" if 32.0 * sectors / samples > 14.0 else "alu/lsu",
-                          "parity": parity}), flush=True)
+                          "slab": vol.vr_get_slab_info(), "parity": parity}), flush=True)
         del out
     vol.close()
 
@@ -526,6 +530,8 @@ def main():
     ap.add_argument("--image", type=int, default=None, help="override the image size (W = H), e.g. 512 for Fig 12's comparison")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-skip", action="store_true", help="vr_set_empty_space_skipping(0): the dense walk (same frames)")
+    ap.add_argument("--slab", type=int, default=None, choices=[0, 1, 2],
+                    help="vr_set_slab_staging: 0 never, 1 auto (library default), 2 whenever the window fits")
     ap.add_argument("--l2-fetch", type=int, default=None, choices=[32, 64, 128],
                     help="device-wide L2 fetch granularity hint in bytes (vr_set_l2_fetch_granularity); default: leave as is")
     ap.add_argument("--sweep", action="store_true", help="run BASELINE.json configs[4] (28 points) instead of the headline")

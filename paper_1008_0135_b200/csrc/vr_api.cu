@@ -285,6 +285,7 @@ struct SlabPlan {
     int dom = 2;
     vr::SlabParams S;
     size_t smem = 0;
+    double bytes_per_sample = 0.0;
     CUtensorMap map;
 };
 
@@ -309,11 +310,9 @@ constexpr size_t SLAB_SMEM_EXTRA = 4096 + 16 + 32 + 16 + 128;   // table, barrie
 
 // Decide whether this frame runs on the slab-staged caster and size its window.  Orthographic frames only: the rays
 // of a CTA tile are parallel, so the window has one size for every tile and slab.
-void plan_slab(const vr_volume* vol, const vr::FrameParams& P, int mode, bool skip_active, SlabPlan& sp) {
+void plan_slab(const vr_volume* vol, const vr::FrameParams& P, SlabPlan& sp) {
     sp.use = false;
     if (vol->slab_mode == 0 || P.proj != VR_PROJ_ORTHO || P.n_runs > 0 || vol->linear_failed) return;
-    if (skip_active && vol->slab_mode != 2) return;          // the skipping caster drops most samples of such frames
-    (void)mode;
     int dom = 0;
     for (int a = 1; a < 3; ++a) if (std::fabs(P.fwd[a]) > std::fabs(P.fwd[dom])) dom = a;
     const double pad[3] = {(double)vr::PAD_X, (double)vr::PAD_Y, (double)vr::PAD_Z};
@@ -368,12 +367,8 @@ void plan_slab(const vr_volume* vol, const vr::FrameParams& P, int mode, bool sk
     S.slot_floats = (int)((fl + 31) & ~31ll);
     sp.smem = (size_t)2 * S.slot_floats * 4 + SLAB_SMEM_EXTRA;
     sp.dom = dom;
-    if (vol->slab_mode == 1) {
-        // auto: only where the frame is on the instruction-bound side of the ridge: window bytes per
-        // sample of a CTA tile below ~16 B (a ray takes D / (|fwd_dom| step) samples per slab)
-        const double samples = (double)vr::CTA_THREADS * D / (std::fabs(P.fwd[dom]) * P.step);
-        if ((double)S.box_floats * 4.0 / samples > 16.0) return;
-    }
+    // window bytes a CTA tile stages per sample it takes (a ray takes D / (|fwd_dom| step) samples per slab)
+    sp.bytes_per_sample = (double)S.box_floats * 4.0 * std::fabs(P.fwd[dom]) * P.step / ((double)vr::CTA_THREADS * D);
     sp.use = true;
 }
 
@@ -443,11 +438,22 @@ vr_status launch_slab(vr_volume* vol, const Frame& f, const SlabPlan& sp, int mo
     return launch_slab_t<vr::MODE_MIP, 2>(vol, f, sp, d_img);
 }
 
-// The product caster of one frame: the slab-staged kernel where plan_slab says so, else the row-cache kernel.
-vr_status cast_frame(vr_volume* vol, const Frame& f, int mode, float* d_img) {
+// Which caster renders this frame, and its per-table / per-volume preparations (mask, linear copy) — called before the
+// frame's timed region.  Measured on config 4 (profiles/r02_slab.md): staging pays when the window bytes per sample
+// are below ~80 against the dense row-cache walk, and below ~130 x (occupied cell fraction) against the skipping
+// caster (40 B per sample for config 3's table, where 31 % of the cells are occupied).
+vr_status choose_caster(vr_volume* vol, const Frame& f, int mode, SlabPlan& sp) {
     const bool skip = skip_applies(vol, mode);
-    SlabPlan sp;
-    plan_slab(vol, f.P, mode, skip, sp);
+    if (skip) {
+        vr_status s = ensure_mask(vol);                                   // builds only after a table change
+        if (s != VR_OK) return s;
+    }
+    plan_slab(vol, f.P, sp);
+    if (sp.use && vol->slab_mode == 1) {
+        const double cells = (double)vol->dims[0] * vol->dims[1] * vol->dims[2];
+        const double limit = skip ? 130.0 * (double)vol->mask_occupied / cells : 80.0;
+        if (sp.bytes_per_sample > limit) sp.use = false;
+    }
     if (sp.use && ensure_linear(vol) != VR_OK) sp.use = false;            // no memory for the second copy: row-cache caster
     if (sp.use) {
         vr_status s = encode_slab_map(vol, sp);
@@ -457,12 +463,12 @@ vr_status cast_frame(vr_volume* vol, const Frame& f, int mode, float* d_img) {
     if (sp.use) {
         vol->last_slab[1] = sp.dom; vol->last_slab[2] = 1 << sp.S.logD;
         for (int a = 0; a < 3; ++a) vol->last_slab[3 + a] = sp.S.w[a];
-        return launch_slab(vol, f, sp, mode, d_img);
     }
-    if (skip) {
-        vr_status s = ensure_mask(vol);                                   // builds only after a table change
-        if (s != VR_OK) return s;
-    }
+    return VR_OK;
+}
+
+vr_status cast_frame(vr_volume* vol, const Frame& f, const SlabPlan& sp, int mode, float* d_img) {
+    if (sp.use) return launch_slab(vol, f, sp, mode, d_img);
     return launch_cast<0>(vol, f, mode, d_img, nullptr, nullptr, nullptr);
 }
 
@@ -682,14 +688,10 @@ vr_status vr_render(vr_volume* vol, const vr_camera* cam, int W, int H, float st
     vol->timed_cast = vol->timed_comp = false;
     if (!direct && (s = ensure_pool(vol, f.pool_pixels * (mode == VR_MODE_EA ? 4 : 1),
                                     (size_t)B * W * H * (mode == VR_MODE_EA ? 4 : 1))) != VR_OK) return s;
-    {   // per-table / per-volume preparations stay outside the timed region of the frame
-        SlabPlan sp;
-        plan_slab(vol, f.P, mode, skip_applies(vol, mode), sp);
-        if (sp.use) ensure_linear(vol);
-        else if (skip_applies(vol, mode) && (s = ensure_mask(vol)) != VR_OK) return s;
-    }
+    SlabPlan sp;
+    if ((s = choose_caster(vol, f, mode, sp)) != VR_OK) return s;
     VR_CUDA(cudaEventRecord(vol->ev[0], vol->stream), "record event");
-    s = cast_frame(vol, f, mode, direct ? d_out_rgba : vol->d_pool);
+    s = cast_frame(vol, f, sp, mode, direct ? d_out_rgba : vol->d_pool);
     if (s != VR_OK) return s;
     VR_CUDA(cudaEventRecord(vol->ev[1], vol->stream), "record event");
     vol->timed_cast = true;
@@ -777,7 +779,9 @@ vr_status vr_render_bricks(vr_volume* vol, const vr_camera* cam, int W, int H, f
     const size_t n = B * (size_t)W * H * (mode == VR_MODE_EA ? 4 : 1);
     vr::fill_kernel<<<1184, 256, 0, vol->stream>>>(d_brick_images, n, mode == VR_MODE_EA ? 0.0f : -INFINITY);
     VR_CUDA(cudaGetLastError(), "fill kernel launch");
-    return cast_frame(vol, f, mode, d_brick_images);
+    SlabPlan sp;
+    if ((s = choose_caster(vol, f, mode, sp)) != VR_OK) return s;
+    return cast_frame(vol, f, sp, mode, d_brick_images);
 }
 
 vr_status vr_composite(vr_volume* vol, const vr_camera* cam, int W, int H, int mode, const float* d_brick_images,

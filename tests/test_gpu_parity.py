@@ -446,6 +446,7 @@ def test_empty_space_skipping_leaves_the_frame_bit_identical(vr, oracle, cfg):
     host = cube.cpu().numpy()
     vol = vr.Volume(cube)
     vol.vr_set_transfer_function(w.table, w.vmin, w.vmax)
+    vol.vr_set_slab_staging(0)          # the statement is about the row-cache caster with and without the mask
     info = vol.vr_get_skip_info()
     assert info["active"] and 0.0 < info["occupied_fraction"] < 0.9 and info["mask_bytes"] > 0, info
     for bricks, proj, step, ert in (((1, 1, 1), wl.PROJ_ORTHO, 1.0, 0.0), ((2, 2, 2), wl.PROJ_PERSP, 0.5, 0.0),
