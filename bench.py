@@ -477,6 +477,11 @@ def run_sweep(args):
         ocam = vro.make_camera(cs.view, cs.projection, cs.fovy_deg, cs.ortho_half_h)
     for pt in wl.sweep_points():
         size, step, mode, bricks = pt["size"], pt["step"], pt["mode"], pt["bricks"]
+        if args.sweep_filter:
+            want = args.sweep_filter.split(":")
+            have = ["MIP" if mode else "EA", str(bricks[0] * bricks[1] * bricks[2]), f"{step:g}", str(size)]
+            if len(want) != 4 or any(a != "*" and a != b for a, b in zip(want, have)):
+                continue
         vol.vr_set_bricks(*bricks)
         out = torch.empty((size, size, 4), dtype=torch.float32, device="cuda")
         for _ in range(3):
@@ -530,6 +535,8 @@ def main():
     ap.add_argument("--image", type=int, default=None, help="override the image size (W = H), e.g. 512 for Fig 12's comparison")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-skip", action="store_true", help="vr_set_empty_space_skipping(0): the dense walk (same frames)")
+    ap.add_argument("--sweep-filter", default=None,
+                    help="with --sweep: run only the points matching MODE:BRICKS:STEP:SIZE (e.g. EA:8:0.25:2048; * = any)")
     ap.add_argument("--slab", type=int, default=None, choices=[0, 1, 2],
                     help="vr_set_slab_staging: 0 never, 1 auto (library default), 2 whenever the window fits")
     ap.add_argument("--l2-fetch", type=int, default=None, choices=[32, 64, 128],

@@ -44,6 +44,10 @@ linearize_kernel(const float* __restrict__ tiled, float* __restrict__ lin, int L
     *reinterpret_cast<float4*>(lin + ((size_t)z * LY + y) * LX + cx * 4) = v;
 }
 
+#ifndef VR_SLAB_WARP_W
+#define VR_SLAB_WARP_W 16
+#endif
+
 struct SlabParams {
     int logD;                 // slab thickness D = 1 << logD cell layers along the dominant axis
     int w[3];                 // window extent in voxels per axis (dominant axis: D + 1; x: + 3 for the aligned start, a multiple of 4)
@@ -118,7 +122,9 @@ cast_slab_kernel(const __grid_constant__ FrameParams P, const __grid_constant__ 
     const int tiles_x = br->tiles_x;
     const int tyi = tloc / tiles_x, txi = tloc - tyi * tiles_x;
     const int warp = tid >> 5, lane = tid & 31;
-    constexpr int WW = VR_WARP_W, WH = 32 / VR_WARP_W, WPR = CTA_W / WW;
+    // warp patch SLAB_WARP_W x (32 / SLAB_WARP_W) pixels: a wide patch spreads the lanes of one pixel row over many
+    // banks of the window (measured 16x2 vs 8x4 in profiles/r02_slab.md)
+    constexpr int WW = VR_SLAB_WARP_W, WH = 32 / VR_SLAB_WARP_W, WPR = CTA_W / WW;
     const int lx = txi * CTA_W + (warp % WPR) * WW + (lane % WW);
     const int ly = tyi * CTA_H + (warp / WPR) * WH + (lane / WW);
     const bool inside = lx < br->rw && ly < br->rh;
