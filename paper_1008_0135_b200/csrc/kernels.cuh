@@ -71,6 +71,31 @@ struct BrickRec {
     int pad;
 };
 
+// Tile order.  Product build: tiles in plain row-major order, tile (tx,ty,tz) at ((tz*TY + ty)*TX + tx).
+// EXPERIMENT -DVR_EXP_MORTON (north_star kernel (1): "Morton-ordered ... tiled layout"; measured and rejected,
+// profiles/r02_experiments.md): macro-blocks of 4x4x4 tiles (32^3 voxels, 128 KB) in row-major order, the 64 tiles of
+// a macro-block in Morton (Z) order: tile-index bits z1 y1 x1 z0 y0 x0.  The address stays separable,
+// off = fx(x) + fy(y) + fz(z); "ty_stride" / "slab_stride" then are the element strides between macro-blocks
+// adjacent in y / z (TX/4 * 32768, TX/4 * TY/4 * 32768) and TX, TY, TZ are multiples of 4.
+#ifdef VR_EXP_MORTON
+__host__ __device__ __forceinline__ unsigned tile_fx(unsigned x) {              // element offset contributed by padded x
+    const unsigned t = x >> 3;
+    return ((t & ~3u) << 13) | ((t & 2u) << 11) | ((t & 1u) << 9) | (x & 7u);
+}
+__host__ __device__ __forceinline__ unsigned tile_fy(unsigned y, unsigned ty_stride) {
+    const unsigned t = y >> 3;
+    return (t >> 2) * ty_stride + (((t & 2u) << 12) | ((t & 1u) << 10) | ((y & 7u) << 3));
+}
+__host__ __device__ __forceinline__ size_t tile_fz(unsigned z, unsigned slab_stride) {
+    const unsigned t = z >> 3;
+    return (size_t)(t >> 2) * slab_stride + (((t & 2u) << 13) | ((t & 1u) << 11) | ((z & 7u) << 6));
+}
+#else
+__host__ __device__ __forceinline__ unsigned tile_fx(unsigned x) { return (x >> 3) * TILE_ELEMS + (x & 7u); }
+__host__ __device__ __forceinline__ unsigned tile_fy(unsigned y, unsigned ty_stride) { return (y >> 3) * ty_stride + ((y & 7u) << 3); }
+__host__ __device__ __forceinline__ size_t tile_fz(unsigned z, unsigned slab_stride) { return (size_t)(z >> 3) * slab_stride + ((z & 7u) << 6); }
+#endif
+
 // ------------------------------------------------------------------------------------------------
 // a0  re-layout.  The tiled copy holds the cube in PADDED coordinates u = voxel index + PAD_a (8, 1, 1): replicated
 // layers below index 0 and at least one above index n-1 on every axis (T_a = ceil((n_a + PAD_a + 1)/8) tiles).  Trilinear
@@ -141,7 +166,12 @@ relayout_kernel(const float* __restrict__ src, float* __restrict__ dst, int nx, 
         }
     }
     const int ntile = min(8, TX - tx0);
+#ifdef VR_EXP_MORTON
+    const unsigned ys = (unsigned)(TX >> 2) * 32768u, zs = ys * (unsigned)(TY >> 2);
+    float* const out_yz = dst + tile_fz((unsigned)tz * 8u, zs) + tile_fy((unsigned)ty * 8u, ys);
+#else
     float4* out = reinterpret_cast<float4*>(dst + ((size_t)((size_t)tz * TY + ty) * TX + tx0) * TILE_ELEMS);
+#endif
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
         const int j = t + 256 * k;           // float4 index inside the 8-tile run
@@ -149,15 +179,18 @@ relayout_kernel(const float* __restrict__ src, float* __restrict__ dst, int nx, 
         if (tile < ntile) {
             const int row = r >> 1, lxq = r & 1;
             const float4 v = *reinterpret_cast<const float4*>(&sm[row][tile * 8 + lxq * 4]);
+#ifdef VR_EXP_MORTON
+            reinterpret_cast<float4*>(out_yz + tile_fx((unsigned)(tx0 + tile) * 8u))[r] = v;
+#else
             out[j] = v;
+#endif
         }
     }
 }
 
 // element offset of PADDED position (x,y,z) = voxel index + (PAD_X, PAD_Y, PAD_Z) in the tiled copy
 __device__ __forceinline__ size_t tiled_index(int x, int y, int z, unsigned ty_stride, unsigned slab_stride) {
-    return (size_t)(z >> 3) * slab_stride + (size_t)(y >> 3) * ty_stride + (size_t)(x >> 3) * TILE_ELEMS +
-           (size_t)(((z & 7) << 6) | ((y & 7) << 3) | (x & 7));
+    return tile_fz((unsigned)z, slab_stride) + (size_t)tile_fy((unsigned)y, ty_stride) + (size_t)tile_fx((unsigned)x);
 }
 
 // NEXT-1  histogram of the cube (the data range and distribution the colour map is built on).
@@ -172,7 +205,16 @@ histogram_kernel(const float* __restrict__ tiled, size_t n_tiles, int TX, int TY
     __syncthreads();
     unsigned nans = 0;
     for (size_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+#ifdef VR_EXP_MORTON
+        const size_t mb = tile >> 6;
+        const unsigned rr = (unsigned)(tile & 63);
+        const int MX = TX >> 2, MY = TY >> 2;
+        const int tx = (int)(mb % MX) * 4 + (int)((rr & 1u) | ((rr >> 2) & 2u));
+        const int ty = (int)((mb / MX) % MY) * 4 + (int)(((rr >> 1) & 1u) | ((rr >> 3) & 2u));
+        const int tz = (int)(mb / ((size_t)MX * MY)) * 4 + (int)(((rr >> 2) & 1u) | ((rr >> 4) & 2u));
+#else
         const int tx = (int)(tile % TX), ty = (int)((tile / TX) % TY), tz = (int)(tile / ((size_t)TX * TY));
+#endif
         const float4* src = reinterpret_cast<const float4*>(tiled + tile * TILE_ELEMS);
         for (int q = threadIdx.x; q < TILE_ELEMS / 4; q += 256) {
             const float4 v4 = __ldcs(src + q);
@@ -308,10 +350,10 @@ __device__ __forceinline__ void fetch_marked(const float* __restrict__ vol, cons
     const unsigned ix = c.ix, iy = c.iy, iz = c.iz;
     // separable tiled offsets; +1 neighbours always exist (padding), see relayout_kernel
     const unsigned ix1 = ix + 1, iy1 = iy + 1, iz1 = iz + 1;
-    const unsigned ex0 = (ix >> 3) * TILE_ELEMS + (ix & 7), ex1 = (ix1 >> 3) * TILE_ELEMS + (ix1 & 7);
-    const unsigned ey0 = (iy >> 3) * P.ty_stride + ((iy & 7) << 3), ey1 = (iy1 >> 3) * P.ty_stride + ((iy1 & 7) << 3);
-    const float* __restrict__ pz0 = vol + (size_t)(iz >> 3) * P.slab_stride + ((iz & 7) << 6);
-    const float* __restrict__ pz1 = vol + (size_t)(iz1 >> 3) * P.slab_stride + ((iz1 & 7) << 6);
+    const unsigned ex0 = tile_fx(ix), ex1 = tile_fx(ix1);
+    const unsigned ey0 = tile_fy(iy, P.ty_stride), ey1 = tile_fy(iy1, P.ty_stride);
+    const float* __restrict__ pz0 = vol + tile_fz(iz, P.slab_stride);
+    const float* __restrict__ pz1 = vol + tile_fz(iz1, P.slab_stride);
     const unsigned e00 = ex0 + ey0, e10 = ex1 + ey0, e01 = ex0 + ey1, e11 = ex1 + ey1;
     F.v[0] = __ldg(pz0 + e00); F.v[1] = __ldg(pz0 + e10);
     F.v[2] = __ldg(pz0 + e01); F.v[3] = __ldg(pz0 + e11);

@@ -145,24 +145,33 @@ __device__ __forceinline__ float sample_cached(unsigned long long vol_base, unsi
     const bool zchg[2] = {wz[0] != K.hz[0], wz[1] != K.hz[1]};
     const bool e_all = !K.straddle;
 
-    const unsigned exc = (cx >> 1) * TILE_ELEMS + ((cx & 1) << 2);
-    const unsigned ey[2] = {(wy[0] >> 3) * ty_stride + ((wy[0] & 7) << 3),
-                            (wy[1] >> 3) * ty_stride + ((wy[1] & 7) << 3)};
+    const unsigned exc = tile_fx(cx << 2);
+    const unsigned ey[2] = {tile_fy(wy[0], ty_stride), tile_fy(wy[1], ty_stride)};
     // Row addresses are formed ONCE, unconditionally (volatile: ptxas otherwise re-derives the whole offset inside
     // each predicated load, +80 instructions per sample); the loads themselves stay predicated.
     unsigned long long rp[2][2];
 #pragma unroll
     for (int b = 0; b < 2; ++b) {
         unsigned long long pz;
+#ifdef VR_EXP_MORTON
+        const unsigned tz_ = wz[b] >> 3;
+        asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(pz) : "r"(tz_ >> 2), "r"(slab_bytes), "l"(vol_base));
+        const unsigned ez = (((tz_ & 2u) << 13) | ((tz_ & 1u) << 11) | ((wz[b] & 7) << 6)) + exc;
+#else
         asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(pz) : "r"(wz[b] >> 3), "r"(slab_bytes), "l"(vol_base));
         const unsigned ez = ((wz[b] & 7) << 6) + exc;
+#endif
 #pragma unroll
         for (int a = 0; a < 2; ++a)
             asm volatile("mad.wide.u32 %0, %1, 4, %2;" : "=l"(rp[a][b]) : "r"(ez + ey[a]), "l"(pz));
     }
     // byte distance from the chunk to voxel ix + 1 when ix is the chunk's last voxel: the next chunk of the same tile
     // row (16 B on) or, from a tile's second chunk, the first voxel of the next tile in x ((512 - 4) * 4 B on)
+#ifdef VR_EXP_MORTON
+    const unsigned de = (ix & 4u) ? (tile_fx((ix | 7u) + 1u) - tile_fx(ix & ~3u)) * 4u : 16u;
+#else
     const unsigned de = (ix & 4u) ? (TILE_ELEMS - 4) * 4u : 16u;
+#endif
 #pragma unroll
     for (int a = 0; a < 2; ++a)
 #pragma unroll

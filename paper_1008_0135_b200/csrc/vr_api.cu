@@ -94,6 +94,10 @@ struct vr_volume {
 
 namespace {
 
+// element strides between tiles (product build) or macro-blocks (-DVR_EXP_MORTON) adjacent in y / z
+unsigned ty_stride_of(const vr_volume* v);
+unsigned slab_stride_of(const vr_volume* v);
+
 struct Frame {                         // everything one frame needs, built on the host
     vr::FrameParams P;
     std::vector<vr::BrickRec> recs;
@@ -101,6 +105,14 @@ struct Frame {                         // everything one frame needs, built on t
     int total_tiles = 0;
     size_t pool_pixels = 0;
 };
+
+#ifdef VR_EXP_MORTON
+unsigned ty_stride_of(const vr_volume* v) { return (unsigned)(v->TX / 4) * 32768u; }
+unsigned slab_stride_of(const vr_volume* v) { return (unsigned)(v->TX / 4) * (unsigned)(v->TY / 4) * 32768u; }
+#else
+unsigned ty_stride_of(const vr_volume* v) { return (unsigned)v->TX * vr::TILE_ELEMS; }
+unsigned slab_stride_of(const vr_volume* v) { return (unsigned)v->TX * (unsigned)v->TY * vr::TILE_ELEMS; }
+#endif
 
 vr_status check_render_args(const vr_volume* vol, const vr_camera* cam, int W, int H, float step, int mode) {
     if (!vol) return fail(VR_ERR_INVALID_ARG, "volume is NULL");
@@ -143,8 +155,8 @@ vr_status build_frame(const vr_volume* vol, const vr_camera* cam, int W, int H, 
     P.step = (double)step;
     P.proj = cam->projection; P.W = W; P.H = H;
     P.nx = vol->dims[0]; P.ny = vol->dims[1]; P.nz = vol->dims[2];
-    P.ty_stride = (unsigned)vol->TX * vr::TILE_ELEMS;
-    P.slab_stride = (unsigned)vol->TX * (unsigned)vol->TY * vr::TILE_ELEMS;
+    P.ty_stride = ty_stride_of(vol);
+    P.slab_stride = slab_stride_of(vol);
     P.vmin = vol->vmin;
     P.inv_range = 1.0f / (vol->vmax - vol->vmin);
     P.ert_on = (ert > 0.0f && ert < 1.0f) ? 1 : 0;
@@ -239,7 +251,7 @@ vr_status ensure_mask(vr_volume* vol) {
     if (e == cudaSuccess) {
         dim3 grid((vol->dims[0] + vr::PAD_X + 31) / 32, (vol->dims[1] + vr::PAD_Y + 7) / 8, (vol->dims[2] + vr::PAD_Z + 7) / 8);
         vr::build_mask_kernel<<<grid, 256, 0, vol->stream>>>(
-            vol->d_tiled, (unsigned)vol->TX * vr::TILE_ELEMS, (unsigned)vol->TX * (unsigned)vol->TY * vr::TILE_ELEMS,
+            vol->d_tiled, ty_stride_of(vol), slab_stride_of(vol),
             vol->dims[0], vol->dims[1], vol->dims[2], key[0], key[1], key[2], vol->d_mask, vol->NBX, vol->NBY,
             vol->d_mask_count);
         e = cudaGetLastError();
@@ -384,8 +396,7 @@ vr_status ensure_linear(vr_volume* vol) {
     if (e == cudaSuccess) {
         dim3 grid((L.LX / 4 + 63) / 64, (L.LY + 3) / 4, L.LZ);
         vr::linearize_kernel<<<grid, 256, 0, vol->stream>>>(vol->d_tiled, vol->d_linear, L.LX, L.LY, L.LZ,
-                                                            (unsigned)vol->TX * vr::TILE_ELEMS,
-                                                            (unsigned)vol->TX * (unsigned)vol->TY * vr::TILE_ELEMS);
+                                                            ty_stride_of(vol), slab_stride_of(vol));
         e = cudaGetLastError();
     }
     if (e == cudaSuccess) e = cudaEventRecord(e1, vol->stream);
@@ -529,7 +540,12 @@ vr_status vr_create_volume(const int dims[3], const float* d_data, vr_volume** o
     }
     // padded: PAD_a replicated layers below, at least one above
     v->TX = (dims[0] + vr::PAD_X + 1 + 7) / 8; v->TY = (dims[1] + vr::PAD_Y + 1 + 7) / 8; v->TZ = (dims[2] + vr::PAD_Z + 1 + 7) / 8;
+#ifdef VR_EXP_MORTON
+    v->TX = (v->TX + 3) & ~3; v->TY = (v->TY + 3) & ~3; v->TZ = (v->TZ + 3) & ~3;   // whole macro-blocks of 4x4x4 tiles
+    if ((double)v->TX * v->TY * 2048.0 >= 1073741824.0) {
+#else
     if ((double)v->TX * v->TY * vr::TILE_ELEMS >= 1073741824.0) {   // slab bytes and in-slab offsets stay 32-bit
+#endif
         delete v;
         return fail(VR_ERR_INVALID_ARG, "vr_create_volume: nx*ny too large for 32-bit in-slab offsets");
     }
@@ -967,8 +983,7 @@ vr_status vr_volume_histogram(vr_volume* vol, int n_bins, float lo, float hi, lo
 vr_status vr_export_linear(vr_volume* vol, float* d_linear) {
     if (!vol || !d_linear) return fail(VR_ERR_INVALID_ARG, "vr_export_linear: NULL argument");
     vr::export_linear_kernel<<<1184, 256, 0, vol->stream>>>(vol->d_tiled, d_linear, vol->dims[0], vol->dims[1],
-                                                             vol->dims[2], (unsigned)vol->TX * vr::TILE_ELEMS,
-                                                             (unsigned)vol->TX * (unsigned)vol->TY * vr::TILE_ELEMS);
+                                                             vol->dims[2], ty_stride_of(vol), slab_stride_of(vol));
     VR_CUDA(cudaGetLastError(), "export kernel launch");
     return VR_OK;
 }
