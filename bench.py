@@ -378,6 +378,7 @@ def run_ours(args):
         "gsamples_evaluated_per_s": evaluated / (total_ms * 1e-3) / 1e9 * world,
         "empty_space_skipping": dict(skip_info, dense=dense),
         "stages_ms": {"cast": cast_total_ms / K, "composite": float(sum(comp_ms)) / K},
+        "caster": {"slab_staged_last_frame": vol.vr_get_slab_info()},
         "relayout": {"ms": relayout_ms, "GBps_read_plus_write": (4.0 * cube.numel() + tiled_bytes) / (relayout_ms * 1e-3) / 1e9
                      if relayout_ms > 0 else None},
         "clocks": clocks,
@@ -466,7 +467,7 @@ def run_sweep(args):
     vol.vr_set_empty_space_skipping(not args.no_skip)
     if args.slab is not None:
         vol.vr_set_slab_staging(args.slab)
-    cs = wl.orbit_camera(w.dims, 30.0, 20.0, wl.PROJ_ORTHO)
+    cs = wl.orbit_camera(w.dims, 30.0, 20.0, wl.PROJ_PERSP if args.sweep_persp else wl.PROJ_ORTHO)
     cam = vr.camera_from_spec(cs)
     peak, peak_src = measured_peak_gbs()
     reps = max(3, min(args.steps, 10))
@@ -511,7 +512,7 @@ def run_sweep(args):
             got = out.cpu().numpy()[py, px]
             parity = {"max_abs_err_vs_oracle": float(np.abs(got - ref["rgba"]).max()), "pixels": int(px.size), "gate": 1e-4}
         print(json.dumps({"sweep_point": {"mode": "MIP" if mode else "EA", "bricks": B, "step_voxels": step,
-                                          "image": f"{size}x{size}"},
+                                          "image": f"{size}x{size}", "projection": "perspective45" if args.sweep_persp else "orthographic"},
                           "ms_per_frame_best": best, "ms_per_frame_median": med, "cast_ms_median": cast_med,
                           "samples": samples, "samples_evaluated": evaluated, "gsamples_per_s": samples / (med * 1e-3) / 1e9,
                           "algorithmic_GB": 32e-9 * sectors, "bytes_per_sample": 32.0 * sectors / samples,
@@ -535,6 +536,7 @@ def main():
     ap.add_argument("--image", type=int, default=None, help="override the image size (W = H), e.g. 512 for Fig 12's comparison")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-skip", action="store_true", help="vr_set_empty_space_skipping(0): the dense walk (same frames)")
+    ap.add_argument("--sweep-persp", action="store_true", help="with --sweep: perspective 45 deg camera instead of the orthographic one")
     ap.add_argument("--sweep-filter", default=None,
                     help="with --sweep: run only the points matching MODE:BRICKS:STEP:SIZE (e.g. EA:8:0.25:2048; * = any)")
     ap.add_argument("--slab", type=int, default=None, choices=[0, 1, 2],

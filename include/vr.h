@@ -115,19 +115,21 @@ vr_status vr_get_skip_info(vr_volume* vol, int* h_active, float* h_build_ms, lon
                            double* h_occupied_fraction);
 
 /* Slab staging (north_star kernel (2): "brick slabs staged through shared memory via TMA where the view is near
- *     axis-aligned"; section 2.4: GPU memory and the per-ray sampling loop).  For ORTHOGRAPHIC
- *     frames the library has a second caster: a CTA marches its 16x8-pixel tile through the brick slab by slab along
- *     the rays' dominant axis; the box of voxels the tile's rays can touch inside a slab is copied into shared memory
- *     by one bulk tensor copy (TMA) from a LINEAR padded copy of the cube (made by the library at the first such
- *     frame: +1 x the cube in device memory, that frame synchronises the stream), and samples are interpolated from
- *     shared memory.  Same lattice, cells, fractions, classification and blending as the other caster (DESIGN.md
- *     O4-O9): frames agree with it to fp32 rounding of the interpolation and both meet the same parity gates.
- *     mode 0: never.  mode 1 (default): orthographic frames without channel mask whose window holds at most ~16 bytes
- *     per sample (dense sampling: small pixel pitch x step), unless empty-space skipping is active for the table.
- *     mode 2: every orthographic frame without channel mask whose window fits shared memory (also when skipping
- *     would apply).  If the linear copy cannot be allocated the library stays on the first caster.
+ *     axis-aligned"; section 2.4: GPU memory and the per-ray sampling loop).  The library has a
+ *     second caster: a CTA marches its 16x8-pixel tile through the brick slab by slab along the dominant axis of the
+ *     view direction; the box of voxels the tile's rays can touch inside a slab is copied into shared memory by one
+ *     bulk tensor copy (TMA) from a LINEAR padded copy of the cube (made by the library at the first such frame: +1 x
+ *     the cube in device memory, that frame synchronises the stream), and samples are interpolated from shared
+ *     memory.  Same lattice, cells, fractions, classification and blending as the other caster (O4-O9):
+ *     frames agree with it to fp32 rounding of the interpolation and both meet the same parity gates.  Frames with a
+ *     channel mask, frames some of whose rays do not advance along the dominant axis (eye inside the cube, very wide
+ *     field of view) and frames whose window does not fit shared memory always use the other caster.
+ *     mode 0: never.  mode 1 (default): when the window stages at most ~80 bytes per sample (dense sampling: small pixel
+ *     pitch x step), ~130 bytes x the occupied-cell fraction when empty-space skipping is active for the table; for
+ *     perspective frames in addition only when four CTAs fit one SM.  mode 2: whenever the window fits.  If the
+ *     linear copy cannot be allocated the library stays on the other caster.
  * vr_get_slab_info: h_info[6] = {last frame used the slab caster, dominant axis, slab thickness D in cell layers,
- *     window extent in voxels along x, y, z}; time of the linear copy in ms; its size in bytes (0: not made).     */
+ *     (largest) window extent in voxels along x, y, z}; time of the linear copy in ms; its size in bytes (0: not made). */
 vr_status vr_set_slab_staging(vr_volume* vol, int mode);
 vr_status vr_get_slab_info(const vr_volume* vol, int h_info[6], float* h_linearize_ms, long long* h_linear_bytes);
 

@@ -48,14 +48,22 @@ linearize_kernel(const float* __restrict__ tiled, float* __restrict__ lin, int L
 #define VR_SLAB_WARP_W 16
 #endif
 
+constexpr int SLAB_MAPS = 4;      // window sizes (tensor maps) a frame may use: perspective windows grow with depth
+
 struct SlabParams {
     int logD;                 // slab thickness D = 1 << logD cell layers along the dominant axis
-    int w[3];                 // window extent in voxels per axis (dominant axis: D + 1; x: + 3 for the aligned start, a multiple of 4)
-    int box_floats;           // w[0]*w[1]*w[2]: what one bulk tensor copy delivers
-    int slot_floats;          // floats per buffer: box_floats rounded up to a multiple of 32 (buffers stay 128-byte aligned)
-    // orthographic rays of a CTA tile: padded position of the ray of pixel (px,py) where its dominant coordinate is c:
-    //   U_a(c) = base_a + px * dpx_a + py * dpy_a + c * slope_a   (a = the two other axes; slope = d_a / d_dom)
-    double base[3], dpx[3], dpy[3], slope[3];
+    int n_maps;               // orthographic: 1; perspective: up to SLAB_MAPS, largest first
+    int w[SLAB_MAPS][3];      // window extent in voxels per axis (dominant axis: D + 1; x: + 3 for the aligned start, a multiple of 4)
+    int box_floats[SLAB_MAPS];// w[k][0]*w[k][1]*w[k][2]: what one bulk tensor copy with map k delivers
+    int slot_floats;          // floats per buffer: box_floats[0] rounded up to a multiple of 32 (buffers stay 128-byte aligned)
+    // The ray of pixel (px,py) in PADDED coordinates, both projections: it passes through Q = q0 + px*dqx + py*dqy with
+    // direction V = v0 + px*dvx + py*dvy (orthographic: Q = the pixel's origin, V = fwd; perspective: Q = the eye,
+    // V = fwd + u T asp right + v T up).  Where its dominant coordinate is c it is at U_a(c) = Q_a + (c - Q_dom) V_a / V_dom.
+    double q0[3], dqx[3], dqy[3], v0[3], dvx[3], dvy[3];
+};
+
+struct SlabMaps {
+    CUtensorMap m[SLAB_MAPS];
 };
 
 // ---- mbarrier / TMA primitives (PTX ISA: mbarrier, cp.async.bulk.tensor) ----
@@ -87,12 +95,13 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, u
 
 // ------------------------------------------------------------------------------------------------
 // a1 + a3 + a4/a5, slab-staged.  Same grid and CTA shape as cast_kernel (16x8-pixel tiles per brick rectangle).
-// DOM = the rays' dominant axis.  Dynamic shared memory: [2 window buffers][256 float4 table][2 mbarriers][origins].
+// DOM = the dominant axis of the view direction.  Dynamic shared memory: [2 window buffers][256 float4 table]
+// [2 mbarriers][corner rays][origins].
 // ------------------------------------------------------------------------------------------------
 template <int MODE, int DOM>
 __global__ void __launch_bounds__(CTA_THREADS)
 cast_slab_kernel(const __grid_constant__ FrameParams P, const __grid_constant__ SlabParams S,
-                 const __grid_constant__ CUtensorMap tmap, const BrickRec* __restrict__ bricks, int n_bricks,
+                 const __grid_constant__ SlabMaps maps, const BrickRec* __restrict__ bricks, int n_bricks,
                  const float4* __restrict__ tf_global, float* __restrict__ img) {
     extern __shared__ unsigned char smem_raw[];
     // carve: windows first (128-byte aligned for the bulk tensor copy)
@@ -100,8 +109,9 @@ cast_slab_kernel(const __grid_constant__ FrameParams P, const __grid_constant__ 
     float* win = reinterpret_cast<float*>(sb);
     float4* tf = reinterpret_cast<float4*>(sb + (size_t)2 * S.slot_floats * 4);
     unsigned long long* bar = reinterpret_cast<unsigned long long*>(tf + 256);
-    int* s_org = reinterpret_cast<int*>(bar + 2);          // [2][4]: window origin per buffer
-    int* s_misc = s_org + 8;                               // [0] brick, [1] min slab, [2] max slab
+    double* s_ray = reinterpret_cast<double*>(bar + 2);    // [4 tile corners][5]: Q_a1, Q_a2, Q_dom, slope_a1, slope_a2
+    int* s_org = reinterpret_cast<int*>(s_ray + 20);       // [2][8]: window origin (3), x pitch, layer pitch per buffer
+    int* s_misc = s_org + 16;                              // [0] brick, [1] min slab, [2] max slab
 
     const int tid = threadIdx.x;
     if (MODE == MODE_EA)
@@ -154,36 +164,57 @@ cast_slab_kernel(const __grid_constant__ FrameParams P, const __grid_constant__ 
     __syncthreads();
     const int s_min = s_misc[1], s_max = s_misc[2];
     const int ns = s_max >= s_min ? s_max - s_min + 1 : 0;
-    const int sgn = P.fwd[DOM] >= 0.0 ? 1 : -1;            // orthographic: every ray has direction fwd
+    const int sgn = P.fwd[DOM] >= 0.0 ? 1 : -1;            // every ray of the frame advances this way along DOM (host check)
     const int s_begin = sgn > 0 ? s_min : s_max;
 
-    // window origin of a slab on the two other axes: min over the tile's corner rays at both faces of the slab
+    // Window of a slab on the two other axes: bounding box of the tile's rays between the slab's faces.  U_a(c) is
+    // linear-fractional in (px,py) and linear in c, so its extremes over the tile are taken by a corner ray on a face.
     constexpr int A1 = (DOM + 1) % 3, A2 = (DOM + 2) % 3;
-    double lo1 = 0.0, lo2 = 0.0;
     if (tid == 0) {
         const int px0 = br->rx0 + txi * CTA_W, py0 = br->ry0 + tyi * CTA_H;
-        lo1 = S.base[A1] + px0 * S.dpx[A1] + py0 * S.dpy[A1] + fmin(0.0, (CTA_W - 1) * S.dpx[A1]) + fmin(0.0, (CTA_H - 1) * S.dpy[A1]);
-        lo2 = S.base[A2] + px0 * S.dpx[A2] + py0 * S.dpy[A2] + fmin(0.0, (CTA_W - 1) * S.dpx[A2]) + fmin(0.0, (CTA_H - 1) * S.dpy[A2]);
+#pragma unroll
+        for (int cnr = 0; cnr < 4; ++cnr) {
+            const double fx = (double)(px0 + ((cnr & 1) ? CTA_W - 1 : 0)), fy = (double)(py0 + ((cnr & 2) ? CTA_H - 1 : 0));
+            const double vd = S.v0[DOM] + fx * S.dvx[DOM] + fy * S.dvy[DOM];
+            s_ray[cnr * 5 + 0] = S.q0[A1] + fx * S.dqx[A1] + fy * S.dqy[A1];
+            s_ray[cnr * 5 + 1] = S.q0[A2] + fx * S.dqx[A2] + fy * S.dqy[A2];
+            s_ray[cnr * 5 + 2] = S.q0[DOM] + fx * S.dqx[DOM] + fy * S.dqy[DOM];
+            s_ray[cnr * 5 + 3] = (S.v0[A1] + fx * S.dvx[A1] + fy * S.dvy[A1]) / vd;
+            s_ray[cnr * 5 + 4] = (S.v0[A2] + fx * S.dvx[A2] + fy * S.dvy[A2]) / vd;
+        }
     }
-    const unsigned box_bytes = (unsigned)S.box_floats * 4u;
     auto issue = [&](int k) {                              // thread 0: start the copy of slab k into buffer k & 1
         const int s = s_begin + sgn * k, slot = k & 1;
         const double c0 = (double)(s << logD), c1 = c0 + (double)(1 << logD);
-        int org[3];
-        org[DOM] = s << logD;
-        org[A1] = (int)floor(lo1 + fmin(c0 * S.slope[A1], c1 * S.slope[A1])) - 1;
-        org[A2] = (int)floor(lo2 + fmin(c0 * S.slope[A2], c1 * S.slope[A2])) - 1;
+        double lo1 = INFINITY, lo2 = INFINITY, hi1 = -INFINITY, hi2 = -INFINITY;
+#pragma unroll
+        for (int cnr = 0; cnr < 4; ++cnr) {
+            const double q1 = s_ray[cnr * 5 + 0], q2 = s_ray[cnr * 5 + 1], qd = s_ray[cnr * 5 + 2];
+            const double m1 = s_ray[cnr * 5 + 3], m2 = s_ray[cnr * 5 + 4];
+            const double a0 = q1 + (c0 - qd) * m1, a1 = q1 + (c1 - qd) * m1;
+            const double b0 = q2 + (c0 - qd) * m2, b1 = q2 + (c1 - qd) * m2;
+            lo1 = fmin(lo1, fmin(a0, a1)); hi1 = fmax(hi1, fmax(a0, a1));
+            lo2 = fmin(lo2, fmin(b0, b1)); hi2 = fmax(hi2, fmax(b0, b1));
+        }
+        int org[3], ext[3];
+        org[DOM] = s << logD; ext[DOM] = 0;
+        org[A1] = (int)floor(lo1) - 1; ext[A1] = (int)floor(hi1) + 3 - org[A1];      // cells up to floor(hi) + 1, + 1 margin
+        org[A2] = (int)floor(lo2) - 1; ext[A2] = (int)floor(hi2) + 3 - org[A2];
+        ext[0] += org[0] & 3;
         org[0] &= ~3;                                      // the copy must start 16-byte aligned (measured: a start
                                                            // coordinate that is not a multiple of 4 floats faults)
-        s_org[slot * 4 + 0] = org[0]; s_org[slot * 4 + 1] = org[1]; s_org[slot * 4 + 2] = org[2];
-        mbar_expect_tx(&bar[slot], box_bytes);
-        tma_load_3d(win + (size_t)slot * S.slot_floats, &tmap, &bar[slot], org[0], org[1], org[2]);
+        int m = 0;                                         // the smallest window that holds the box (map 0 always does)
+        for (int q = 1; q < S.n_maps; ++q)
+            if (ext[A1] <= S.w[q][A1] && ext[A2] <= S.w[q][A2]) m = q;
+        int* so = s_org + slot * 8;
+        so[0] = org[0]; so[1] = org[1]; so[2] = org[2]; so[3] = S.w[m][0]; so[4] = S.w[m][0] * S.w[m][1];
+        mbar_expect_tx(&bar[slot], (unsigned)S.box_floats[m] * 4u);
+        tma_load_3d(win + (size_t)slot * S.slot_floats, &maps.m[m], &bar[slot], org[0], org[1], org[2]);
     };
     if (tid == 0 && ns > 0) issue(0);
 
     float Cr = 0.f, Cg = 0.f, Cb = 0.f, A = 0.f, M = -INFINITY;
     int j = 0;
-    const int w0 = S.w[0], w01 = S.w[0] * S.w[1];
     for (int k = 0; k < ns; ++k) {
         const int slot = k & 1;
         const int any = __syncthreads_or(j < n);           // every thread is done with slab k - 1 (buffer (k + 1) & 1)
@@ -191,8 +222,9 @@ cast_slab_kernel(const __grid_constant__ FrameParams P, const __grid_constant__ 
         mbar_wait(&bar[slot], (unsigned)(k >> 1) & 1u);    // slab k has landed (it was issued in any case)
         if (!any) break;
         const int s = s_begin + sgn * k;
+        const int w0 = s_org[slot * 8 + 3], w01 = s_org[slot * 8 + 4];
         const float* __restrict__ wbase = win + (size_t)slot * S.slot_floats
-                                          - (s_org[slot * 4 + 0] + s_org[slot * 4 + 1] * w0 + s_org[slot * 4 + 2] * w01);
+                                          - (s_org[slot * 8 + 0] + s_org[slot * 8 + 1] * w0 + s_org[slot * 8 + 2] * w01);
         while (j < n) {
             int jl = j - js;
             if (jl == P.seg_len) {

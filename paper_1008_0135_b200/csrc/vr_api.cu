@@ -291,14 +291,14 @@ vr_status launch_cast(vr_volume* vol, const Frame& f, int mode, float* d_img, un
     return VR_OK;
 }
 
-// ---- slab-staged caster (slab.cuh): eligibility, window sizing, tensor map, launch ----
+// ---- slab-staged caster (slab.cuh): eligibility, window sizing, tensor maps, launch ----
 struct SlabPlan {
     bool use = false;
     int dom = 2;
     vr::SlabParams S;
     size_t smem = 0;
     double bytes_per_sample = 0.0;
-    CUtensorMap map;
+    vr::SlabMaps maps;
 };
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -318,69 +318,150 @@ EncodeTiledFn encode_tiled_fn() {
     return fn;
 }
 
-constexpr size_t SLAB_SMEM_EXTRA = 4096 + 16 + 32 + 16 + 128;   // table, barriers, origins, misc, alignment slack
+constexpr size_t SLAB_SMEM_EXTRA = 4096 + 16 + 160 + 64 + 16 + 128;   // table, barriers, corner rays, origins, misc, slack
 
-// Decide whether this frame runs on the slab-staged caster and size its window.  Orthographic frames only: the rays
-// of a CTA tile are parallel, so the window has one size for every tile and slab.
-void plan_slab(const vr_volume* vol, const vr::FrameParams& P, SlabPlan& sp) {
+// Largest extent (voxels, before margins) of a slab window on the two non-dominant axes over every CTA tile of the
+// frame and every slab of its brick, for slabs of D cell layers.  false: some ray of the frame does not advance along
+// the dominant axis in the direction of fwd, or is too oblique to it (perspective), or there are too many tiles to scan.
+bool slab_extents(const Frame& f, const vr::SlabParams& S, int dom, int D, double ext[3]) {
+    const vr::FrameParams& P = f.P;
+    const int a1 = (dom + 1) % 3, a2 = (dom + 2) % 3;
+    const double pad[3] = {(double)vr::PAD_X, (double)vr::PAD_Y, (double)vr::PAD_Z};
+    const double sg = P.fwd[dom] >= 0.0 ? 1.0 : -1.0;
+    ext[0] = ext[1] = ext[2] = 0.0;
+    if (P.proj == VR_PROJ_PERSP && f.total_tiles > 400000) return false;
+    for (const vr::BrickRec& r : f.recs) {
+        if (r.rw <= 0 || r.rh <= 0) continue;
+        const double cmin = (double)r.lo[dom] + pad[dom] - 1.0, cmax = (double)r.hi[dom] + pad[dom] + 1.0;
+        const int tiles_x = (r.rw + vr::CTA_W - 1) / vr::CTA_W, tiles_y = (r.rh + vr::CTA_H - 1) / vr::CTA_H;
+        const int nty = P.proj == VR_PROJ_PERSP ? tiles_y : 1, ntx = P.proj == VR_PROJ_PERSP ? tiles_x : 1;   // orthographic: every tile alike
+        for (int ty = 0; ty < nty; ++ty)
+            for (int tx = 0; tx < ntx; ++tx) {
+                double q[4][3], m[4][2];
+                for (int c = 0; c < 4; ++c) {
+                    const double fx = (double)(r.rx0 + tx * vr::CTA_W + ((c & 1) ? vr::CTA_W - 1 : 0));
+                    const double fy = (double)(r.ry0 + ty * vr::CTA_H + ((c & 2) ? vr::CTA_H - 1 : 0));
+                    const double vd = S.v0[dom] + fx * S.dvx[dom] + fy * S.dvy[dom];
+                    if (!(vd * sg > 1e-9)) return false;
+                    q[c][0] = S.q0[a1] + fx * S.dqx[a1] + fy * S.dqy[a1];
+                    q[c][1] = S.q0[a2] + fx * S.dqx[a2] + fy * S.dqy[a2];
+                    q[c][2] = S.q0[dom] + fx * S.dqx[dom] + fy * S.dqy[dom];
+                    m[c][0] = (S.v0[a1] + fx * S.dvx[a1] + fy * S.dvy[a1]) / vd;
+                    m[c][1] = (S.v0[a2] + fx * S.dvx[a2] + fy * S.dvy[a2]) / vd;
+                    if (std::fabs(m[c][0]) > 4.0 || std::fabs(m[c][1]) > 4.0) return false;
+                }
+                // the extent is convex in the slab position: its maximum over the brick is at the first or the last slab
+                for (int end = 0; end < 2; ++end) {
+                    const double c0 = end == 0 ? cmin - D + 1.0 : cmax - 1.0, c1 = c0 + D;    // slabs overhanging the brick's ends
+                    for (int k = 0; k < 2; ++k) {
+                        double lo = INFINITY, hi = -INFINITY;
+                        for (int c = 0; c < 4; ++c) {
+                            const double u0 = q[c][k] + (c0 - q[c][2]) * m[c][k], u1 = q[c][k] + (c1 - q[c][2]) * m[c][k];
+                            lo = std::min(lo, std::min(u0, u1)); hi = std::max(hi, std::max(u0, u1));
+                        }
+                        const int a = k == 0 ? a1 : a2;
+                        ext[a] = std::max(ext[a], hi - lo);
+                    }
+                }
+            }
+    }
+    return true;
+}
+
+// Decide whether this frame can run on the slab-staged caster and size its windows.
+void plan_slab(const vr_volume* vol, const Frame& f, double limit_bytes_per_sample, SlabPlan& sp) {
+    const vr::FrameParams& P = f.P;
     sp.use = false;
-    if (vol->slab_mode == 0 || P.proj != VR_PROJ_ORTHO || P.n_runs > 0 || vol->linear_failed) return;
+    if (vol->slab_mode == 0 || P.n_runs > 0 || vol->linear_failed || f.total_tiles == 0) return;
     int dom = 0;
     for (int a = 1; a < 3; ++a) if (std::fabs(P.fwd[a]) > std::fabs(P.fwd[dom])) dom = a;
     const double pad[3] = {(double)vr::PAD_X, (double)vr::PAD_Y, (double)vr::PAD_Z};
-    double q0[3], dqx[3], dqy[3];                            // padded position of the pixel's ray origin, affine in (px,py)
-    for (int a = 0; a < 3; ++a) {
-        q0[a] = P.eye[a] + (1.0 / P.W - 1.0) * P.h * P.asp * P.right[a] + (1.0 / P.H - 1.0) * P.h * P.up[a] + pad[a] - 0.5;
-        dqx[a] = 2.0 * P.h * P.asp * P.right[a] / P.W;
-        dqy[a] = 2.0 * P.h * P.up[a] / P.H;
-    }
     vr::SlabParams& S = sp.S;
     for (int a = 0; a < 3; ++a) {
-        S.slope[a] = P.fwd[a] / P.fwd[dom];
-        S.base[a] = q0[a] - q0[dom] * S.slope[a];
-        S.dpx[a] = dqx[a] - dqx[dom] * S.slope[a];
-        S.dpy[a] = dqy[a] - dqy[dom] * S.slope[a];
+        if (P.proj == VR_PROJ_ORTHO) {
+            S.q0[a] = P.eye[a] + (1.0 / P.W - 1.0) * P.h * P.asp * P.right[a] + (1.0 / P.H - 1.0) * P.h * P.up[a] + pad[a] - 0.5;
+            S.dqx[a] = 2.0 * P.h * P.asp * P.right[a] / P.W;
+            S.dqy[a] = 2.0 * P.h * P.up[a] / P.H;
+            S.v0[a] = P.fwd[a]; S.dvx[a] = 0.0; S.dvy[a] = 0.0;
+        } else {
+            S.q0[a] = P.eye[a] + pad[a] - 0.5; S.dqx[a] = 0.0; S.dqy[a] = 0.0;
+            S.v0[a] = P.fwd[a] + (1.0 / P.W - 1.0) * P.tanhalf * P.asp * P.right[a] + (1.0 / P.H - 1.0) * P.tanhalf * P.up[a];
+            S.dvx[a] = 2.0 * P.tanhalf * P.asp * P.right[a] / P.W;
+            S.dvy[a] = 2.0 * P.tanhalf * P.up[a] / P.H;
+        }
     }
-    int best = -1;
+    if (P.proj == VR_PROJ_PERSP && std::isfinite(limit_bytes_per_sample)) {
+        // Quick reject before the scan over all tiles (a frame of the headline has ~10^4 of them): the tile at the image
+        // centre, half way through the cube, in a slab one cell layer thick, already stages more bytes per sample than
+        // the limit (d(V_a/V_dom)/dpx = (dvx_a V_dom - dvx_dom V_a) / V_dom^2).
+        const double fx = 0.5 * P.W, fy = 0.5 * P.H;
+        const double vd = S.v0[dom] + fx * S.dvx[dom] + fy * S.dvy[dom];
+        const double dims[3] = {(double)P.nx, (double)P.ny, (double)P.nz};
+        const double depth = std::fabs(0.5 * dims[dom] + pad[dom] - S.q0[dom]);
+        double e[3] = {0.0, 0.0, 0.0};
+        for (int a = 0; a < 3; ++a) {
+            const double va = S.v0[a] + fx * S.dvx[a] + fy * S.dvy[a];
+            e[a] = depth * (std::fabs(S.dvx[a] * vd - S.dvx[dom] * va) * (vr::CTA_W - 1) +
+                            std::fabs(S.dvy[a] * vd - S.dvy[dom] * va) * (vr::CTA_H - 1)) / (vd * vd);
+        }
+        double wq[3];
+        for (int a = 0; a < 3; ++a) wq[a] = e[a] + (a == 0 ? 8.0 : 5.0);             // the margins of window_scan
+        const double layer = wq[(dom + 1) % 3] * wq[(dom + 2) % 3] * 4.0;            // bytes per cell layer of the window
+        const double layers = std::floor(113.0 * 1024.0 / (2.0 * layer));            // what two buffers can hold
+        if (layers < 2.0) return;
+        const double Dq = layers >= 9.0 ? 8.0 : layers >= 5.0 ? 4.0 : layers >= 3.0 ? 2.0 : 1.0;
+        const double low = layer * (Dq + 1.0) / Dq * std::fabs(P.fwd[dom]) * P.step / (double)vr::CTA_THREADS;
+        if (low > limit_bytes_per_sample) return;
+    }
+    auto window_scan = [&](int logd, int w[3]) -> bool {
+        const int D = 1 << logd;
+        double ext[3];
+        if (!slab_extents(f, S, dom, D, ext)) return false;
+        for (int a = 0; a < 3; ++a) {
+            w[a] = a == dom ? D + 1 : (int)std::ceil(ext[a]) + 5;
+            if (a == 0) w[a] = (w[a] + 3 + 3) & ~3;          // + 3: the copy starts at a multiple of 4 voxels
+            if (w[a] > 256) return false;
+        }
+        return true;
+    };
+    bool have[4] = {false, false, false, false}, okw[4] = {false, false, false, false};
+    int wc[4][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+    auto window = [&](int logd, int w[3]) -> bool {           // one scan per slab thickness
+        if (!have[logd]) { have[logd] = true; okw[logd] = window_scan(logd, wc[logd]); }
+        for (int a = 0; a < 3; ++a) w[a] = wc[logd][a];
+        return okw[logd];
+    };
+    int best = -1, w[3] = {0, 0, 0};
     for (int pass = 0; pass < 2 && best < 0; ++pass) {
         const size_t budget = pass == 0 ? (size_t)56 * 1024 : (size_t)113 * 1024;   // 4 or 2 CTAs per SM
         for (int logd = 3; logd >= 0; --logd) {
             if (vol->slab_logd >= 0 && logd != vol->slab_logd) continue;
-            const int D = 1 << logd;
-            long long fl = 1;
-            bool fits = true;
-            for (int a = 0; a < 3; ++a) {
-                int w;
-                if (a == dom) w = D + 1;
-                else w = (int)std::ceil((vr::CTA_W - 1) * std::fabs(S.dpx[a]) + (vr::CTA_H - 1) * std::fabs(S.dpy[a]) +
-                                        D * std::fabs(S.slope[a])) + 5;
-                if (a == 0) w = (w + 3 + 3) & ~3;          // + 3: the copy starts at a multiple of 4 voxels
-                if (w > 256) fits = false;
-                fl *= w;
-            }
+            if (!window(logd, w)) continue;
+            const long long fl = (long long)w[0] * w[1] * w[2];
             const size_t smem = (size_t)2 * (size_t)((fl + 31) & ~31ll) * 4 + SLAB_SMEM_EXTRA;
-            if (fits && smem <= budget) { best = logd; break; }
+            if (smem <= budget) { best = logd; break; }
         }
     }
     if (best < 0) return;
     const int D = 1 << best;
     S.logD = best;
-    long long fl = 1;
-    for (int a = 0; a < 3; ++a) {
-        int w;
-        if (a == dom) w = D + 1;
-        else w = (int)std::ceil((vr::CTA_W - 1) * std::fabs(S.dpx[a]) + (vr::CTA_H - 1) * std::fabs(S.dpy[a]) +
-                                D * std::fabs(S.slope[a])) + 5;
-        if (a == 0) w = (w + 3 + 3) & ~3;          // + 3: the copy starts at a multiple of 4 voxels
-        S.w[a] = w;
-        fl *= w;
+    S.n_maps = P.proj == VR_PROJ_PERSP ? vr::SLAB_MAPS : 1;
+    const int a1 = (dom + 1) % 3, a2 = (dom + 2) % 3;
+    for (int k = 0; k < vr::SLAB_MAPS; ++k) {
+        const double fk = std::pow(0.8, (double)k);          // perspective: windows near the eye are smaller
+        for (int a = 0; a < 3; ++a) S.w[k][a] = w[a];
+        if (k > 0 && k < S.n_maps) {
+            S.w[k][a1] = std::max(8, (int)std::ceil(w[a1] * fk));
+            S.w[k][a2] = std::max(8, (int)std::ceil(w[a2] * fk));
+            S.w[k][0] = std::min(w[0], (S.w[k][0] + 3) & ~3);
+        }
+        S.box_floats[k] = S.w[k][0] * S.w[k][1] * S.w[k][2];
     }
-    S.box_floats = (int)fl;
-    S.slot_floats = (int)((fl + 31) & ~31ll);
+    S.slot_floats = (S.box_floats[0] + 31) & ~31;
     sp.smem = (size_t)2 * S.slot_floats * 4 + SLAB_SMEM_EXTRA;
     sp.dom = dom;
-    // window bytes a CTA tile stages per sample it takes (a ray takes D / (|fwd_dom| step) samples per slab)
-    sp.bytes_per_sample = (double)S.box_floats * 4.0 * std::fabs(P.fwd[dom]) * P.step / ((double)vr::CTA_THREADS * D);
+    // window bytes a CTA tile stages per sample it takes (a ray takes about D / (|fwd_dom| step) samples per slab)
+    sp.bytes_per_sample = (double)S.box_floats[0] * 4.0 * std::fabs(P.fwd[dom]) * P.step / ((double)vr::CTA_THREADS * D);
     sp.use = true;
 }
 
@@ -414,12 +495,15 @@ vr_status encode_slab_map(vr_volume* vol, SlabPlan& sp) {
     const vr::LinearDims L = vr::linear_dims(vol->dims[0], vol->dims[1], vol->dims[2]);
     const cuuint64_t gdim[3] = {(cuuint64_t)L.LX, (cuuint64_t)L.LY, (cuuint64_t)L.LZ};
     const cuuint64_t gstr[2] = {(cuuint64_t)L.LX * 4, (cuuint64_t)L.LX * L.LY * 4};
-    const cuuint32_t box[3] = {(cuuint32_t)sp.S.w[0], (cuuint32_t)sp.S.w[1], (cuuint32_t)sp.S.w[2]};
     const cuuint32_t estr[3] = {1, 1, 1};
-    const CUresult r = enc(&sp.map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, vol->d_linear, gdim, gstr, box, estr,
-                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) return fail(VR_ERR_CUDA, "cuTensorMapEncodeTiled failed (code " + std::to_string((int)r) + ")");
+    for (int k = 0; k < vr::SLAB_MAPS; ++k) {
+        const int kk = k < sp.S.n_maps ? k : 0;
+        const cuuint32_t box[3] = {(cuuint32_t)sp.S.w[kk][0], (cuuint32_t)sp.S.w[kk][1], (cuuint32_t)sp.S.w[kk][2]};
+        const CUresult r = enc(&sp.maps.m[k], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, vol->d_linear, gdim, gstr, box, estr,
+                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return fail(VR_ERR_CUDA, "cuTensorMapEncodeTiled failed (code " + std::to_string((int)r) + ")");
+    }
     return VR_OK;
 }
 
@@ -432,7 +516,7 @@ vr_status launch_slab_t(vr_volume* vol, const Frame& f, const SlabPlan& sp, floa
         attr_set = true;
     }
     vr::cast_slab_kernel<MODE, DOM><<<f.total_tiles, vr::CTA_THREADS, sp.smem, vol->stream>>>(
-        f.P, sp.S, sp.map, vol->d_bricks, (int)f.recs.size(), vol->d_tf_ea, d_img);
+        f.P, sp.S, sp.maps, vol->d_bricks, (int)f.recs.size(), vol->d_tf_ea, d_img);
     VR_CUDA(cudaGetLastError(), "slab caster launch");
     return VR_OK;
 }
@@ -459,12 +543,16 @@ vr_status choose_caster(vr_volume* vol, const Frame& f, int mode, SlabPlan& sp) 
         vr_status s = ensure_mask(vol);                                   // builds only after a table change
         if (s != VR_OK) return s;
     }
-    plan_slab(vol, f.P, sp);
-    if (sp.use && vol->slab_mode == 1) {
+    double limit = INFINITY;                                              // mode 2: whenever the window fits
+    if (vol->slab_mode == 1) {
         const double cells = (double)vol->dims[0] * vol->dims[1] * vol->dims[2];
-        const double limit = skip ? 130.0 * (double)vol->mask_occupied / cells : 80.0;
-        if (sp.bytes_per_sample > limit) sp.use = false;
+        limit = skip ? 130.0 * (double)vol->mask_occupied / cells : 80.0;
     }
+    plan_slab(vol, f, limit, sp);
+    if (sp.use && sp.bytes_per_sample > limit) sp.use = false;
+    // perspective windows are sized for the far corner of the frame: measured on config 3's cube (profiles/r02_slab.md)
+    // they only pay when four CTAs still fit an SM
+    if (sp.use && vol->slab_mode == 1 && f.P.proj == VR_PROJ_PERSP && sp.smem > (size_t)56 * 1024) sp.use = false;
     if (sp.use && ensure_linear(vol) != VR_OK) sp.use = false;            // no memory for the second copy: row-cache caster
     if (sp.use) {
         vr_status s = encode_slab_map(vol, sp);
@@ -473,7 +561,7 @@ vr_status choose_caster(vr_volume* vol, const Frame& f, int mode, SlabPlan& sp) 
     vol->last_slab[0] = sp.use ? 1 : 0;
     if (sp.use) {
         vol->last_slab[1] = sp.dom; vol->last_slab[2] = 1 << sp.S.logD;
-        for (int a = 0; a < 3; ++a) vol->last_slab[3 + a] = sp.S.w[a];
+        for (int a = 0; a < 3; ++a) vol->last_slab[3 + a] = sp.S.w[0][a];
     }
     return VR_OK;
 }

@@ -136,9 +136,6 @@ def test_slab_caster_not_used_where_it_does_not_apply(vr):
     cube = w.cube("cuda")
     vol = vr.Volume(cube)
     vol.vr_set_transfer_function(w.table, w.vmin, w.vmax)
-    csp = wl.orbit_camera(w.dims, 30.0, 20.0, wl.PROJ_PERSP)
-    _, _, info = render(vr, vol, csp, 64, 64, 0.5, 0, 0.0, 2)
-    assert not info["used"]                                               # perspective frames: row-cache caster
     cs = w.camera()
     mask = np.ones(w.dims[2], dtype=np.uint8)
     mask[10:20] = 0
@@ -148,4 +145,60 @@ def test_slab_caster_not_used_where_it_does_not_apply(vr):
     vol.vr_set_channel_mask(None)
     _, _, info = render(vr, vol, cs, 64, 64, 0.5, 0, 0.0, 0)
     assert not info["used"]
+    vol.close()
+
+
+PVIEWS = [(30.0, 20.0), (215.0, -10.0), (95.0, 15.0), (10.0, 75.0), (0.0, 0.0)]
+
+
+@pytest.mark.parametrize("az,el", PVIEWS)
+def test_slab_caster_perspective_matches_oracle(vr, oracle, az, el):
+    """Perspective frames: the window of a slab follows the diverging rays (several window sizes per frame)."""
+    dims = (72, 50, 41)
+    cube = noisy_cube(dims, 13)
+    table = wl.tf_ramp(0.06)
+    vmin, vmax = -3.0, 9.0
+    vol = vr.Volume(cube)
+    vol.vr_set_transfer_function(table, vmin, vmax)
+    cs = wl.orbit_camera(dims, az, el, wl.PROJ_PERSP)
+    W, H = 200, 170
+    for bricks, step, ert in [((1, 1, 1), 0.5, 0.0), ((2, 2, 1), 0.25, 0.0), ((2, 3, 2), 0.5, 0.995)]:
+        vol.vr_set_bricks(*bricks)
+        got, _, info = render(vr, vol, cs, W, H, step, 0, ert, 2)
+        assert info["used"], info
+        ref = oracle.render(cube.cpu().numpy(), table, vmin, vmax, bricks, ocam(oracle, cs), W, H, step, 0, ert, route=1)["rgba"]
+        err = np.abs(got - ref).max()
+        assert err <= (TOL_ERT if ert > 0 else TOL_EA), (bricks, step, ert, err)
+        assert ref[..., 3].max() > 0.3
+        other, _, info0 = render(vr, vol, cs, W, H, step, 0, ert, 0)
+        assert not info0["used"]
+        if ert == 0:
+            assert np.abs(got - other).max() <= 2e-5
+    got, sc, info = render(vr, vol, cs, W, H, 0.5, 1, 0.0, 2, want_scalar=True)
+    assert info["used"]
+    ref = oracle.render(cube.cpu().numpy(), table, vmin, vmax, (2, 3, 2), ocam(oracle, cs), W, H, 0.5, 1, 0.0, route=0)
+    m = ref["scalar"]
+    hit = np.isfinite(m)
+    assert (np.isfinite(sc) == hit).all()
+    assert (np.abs(sc[hit] - m[hit]) <= 1e-4 * np.maximum(1.0, np.abs(m[hit]))).all()
+    vol.close()
+
+
+def test_slab_caster_perspective_eye_inside_or_wide(vr, oracle):
+    """An eye inside the cube and a very wide field of view: rays that do not advance along the dominant axis make the
+    frame ineligible (row-cache caster); either way the frame matches the oracle."""
+    import dataclasses
+    dims = (48, 40, 36)
+    cube = noisy_cube(dims, 14)
+    table = wl.tf_ramp(0.1)
+    vol = vr.Volume(cube)
+    vol.vr_set_transfer_function(table, -3.0, 9.0)
+    vol.vr_set_bricks(2, 2, 2)
+    eye = (20.0, 18.0, 15.0)
+    view = wl.look_at(eye, (40.0, 30.0, 30.0))
+    for fov in (45.0, 150.0):
+        cs = wl.CameraSpec(view=view, projection=wl.PROJ_PERSP, fovy_deg=fov, ortho_half_h=1.0)
+        got, _, info = render(vr, vol, cs, 96, 80, 0.5, 0, 0.0, 2)
+        ref = oracle.render(cube.cpu().numpy(), table, -3.0, 9.0, (2, 2, 2), ocam(oracle, cs), 96, 80, 0.5, 0, 0.0, route=0)["rgba"]
+        assert np.abs(got - ref).max() <= TOL_EA, (fov, info)
     vol.close()
