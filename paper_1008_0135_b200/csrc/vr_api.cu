@@ -550,6 +550,10 @@ vr_status choose_caster(vr_volume* vol, const Frame& f, int mode, SlabPlan& sp) 
     }
     plan_slab(vol, f, limit, sp);
     if (sp.use && sp.bytes_per_sample > limit) sp.use = false;
+    // Views whose dominant axis is x (the fastest axis in memory): a slab is then a few voxels thick along the rows, the
+    // copy degenerates into hundreds of 32-48-byte rows and the window's bank mapping into 8-way conflicts: measured
+    // 3.3-5.1 ms against 2.3 ms on config 5 (profiles/r02_slab.md).  Such frames stay on the row-cache caster.
+    if (sp.use && vol->slab_mode == 1 && sp.dom == 0) sp.use = false;
     // perspective windows are sized for the far corner of the frame: measured on config 3's cube (profiles/r02_slab.md)
     // they only pay when four CTAs still fit an SM
     if (sp.use && vol->slab_mode == 1 && f.P.proj == VR_PROJ_PERSP && sp.smem > (size_t)56 * 1024) sp.use = false;
