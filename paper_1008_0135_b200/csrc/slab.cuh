@@ -48,6 +48,7 @@ linearize_kernel(const float* __restrict__ tiled, float* __restrict__ lin, int L
 #define VR_SLAB_WARP_W 16
 #endif
 
+constexpr double SLAB_FUZZ = 1e-3;
 constexpr int SLAB_MAPS = 4;      // window sizes (tensor maps) a frame may use: perspective windows grow with depth
 
 struct SlabParams {
@@ -198,8 +199,10 @@ cast_slab_kernel(const __grid_constant__ FrameParams P, const __grid_constant__ 
         }
         int org[3], ext[3];
         org[DOM] = s << logD; ext[DOM] = 0;
-        org[A1] = (int)floor(lo1) - 1; ext[A1] = (int)floor(hi1) + 3 - org[A1];      // cells up to floor(hi) + 1, + 1 margin
-        org[A2] = (int)floor(lo2) - 1; ext[A2] = (int)floor(hi2) + 3 - org[A2];
+        // voxels floor(lo) .. floor(hi) + 1; SLAB_FUZZ covers the difference between these fp64 corner rays and the
+        // fp32 segment arithmetic that places the samples (<= 1e-5 voxel)
+        org[A1] = (int)floor(lo1 - SLAB_FUZZ); ext[A1] = (int)floor(hi1 + SLAB_FUZZ) + 2 - org[A1];
+        org[A2] = (int)floor(lo2 - SLAB_FUZZ); ext[A2] = (int)floor(hi2 + SLAB_FUZZ) + 2 - org[A2];
         ext[0] += org[0] & 3;
         org[0] &= ~3;                                      // the copy must start 16-byte aligned (measured: a start
                                                            // coordinate that is not a multiple of 4 floats faults)

@@ -405,7 +405,7 @@ void plan_slab(const vr_volume* vol, const Frame& f, double limit_bytes_per_samp
                             std::fabs(S.dvy[a] * vd - S.dvy[dom] * va) * (vr::CTA_H - 1)) / (vd * vd);
         }
         double wq[3];
-        for (int a = 0; a < 3; ++a) wq[a] = e[a] + (a == 0 ? 8.0 : 5.0);             // the margins of window_scan
+        for (int a = 0; a < 3; ++a) wq[a] = e[a] + (a == 0 ? 5.0 : 2.0);             // the margins of window_scan
         const double layer = wq[(dom + 1) % 3] * wq[(dom + 2) % 3] * 4.0;            // bytes per cell layer of the window
         const double layers = std::floor(113.0 * 1024.0 / (2.0 * layer));            // what two buffers can hold
         if (layers < 2.0) return;
@@ -418,7 +418,7 @@ void plan_slab(const vr_volume* vol, const Frame& f, double limit_bytes_per_samp
         double ext[3];
         if (!slab_extents(f, S, dom, D, ext)) return false;
         for (int a = 0; a < 3; ++a) {
-            w[a] = a == dom ? D + 1 : (int)std::ceil(ext[a]) + 5;
+            w[a] = a == dom ? D + 1 : (int)std::ceil(ext[a] + 2.0 * vr::SLAB_FUZZ) + 2;   // the kernel's floor(hi + fuzz) + 2 - floor(lo - fuzz)
             if (a == 0) w[a] = (w[a] + 3 + 3) & ~3;          // + 3: the copy starts at a multiple of 4 voxels
             if (w[a] > 256) return false;
         }
