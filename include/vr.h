@@ -118,9 +118,10 @@ vr_status vr_get_skip_info(vr_volume* vol, int* h_active, float* h_build_ms, lon
  *     axis-aligned"; section 2.4: GPU memory and the per-ray sampling loop).  The library has a
  *     second caster: a CTA marches its 16x8-pixel tile through the brick slab by slab along the dominant axis of the
  *     view direction; the box of voxels the tile's rays can touch inside a slab is copied into shared memory by one
- *     bulk tensor copy (TMA) from a LINEAR padded copy of the cube (made by the library at the first such frame: +1 x
- *     the cube in device memory, that frame synchronises the stream), and samples are interpolated from shared
- *     memory.  Same lattice, cells, fractions, classification and blending as the other caster (O4-O9):
+ *     bulk tensor copy (TMA) from a LINEAR padded copy of the cube (made by the library at the first such frame and
+ *     kept: x fastest for views whose dominant axis is y or z, a second one with z fastest for views whose dominant
+ *     axis is x; + 1 x the cube in device memory each, the frame that makes one synchronises the stream), and samples
+ *     are interpolated from shared memory.  Same lattice, cells, fractions, classification and blending as the other caster (O4-O9):
  *     frames agree with it to fp32 rounding of the interpolation and both meet the same parity gates.  Frames with a
  *     channel mask, frames some of whose rays do not advance along the dominant axis (eye inside the cube, very wide
  *     field of view) and frames whose window does not fit shared memory always use the other caster.
@@ -129,7 +130,8 @@ vr_status vr_get_skip_info(vr_volume* vol, int* h_active, float* h_build_ms, lon
  *     perspective frames in addition only when four CTAs fit one SM.  mode 2: whenever the window fits.  If the
  *     linear copy cannot be allocated the library stays on the other caster.
  * vr_get_slab_info: h_info[6] = {last frame used the slab caster, dominant axis, slab thickness D in cell layers,
- *     (largest) window extent in voxels along x, y, z}; time of the linear copy in ms; its size in bytes (0: not made). */
+ *     (largest) window extent in voxels along x, y, z}; time spent making the linear copies in ms; their size in bytes
+ *     (0: none made). */
 vr_status vr_set_slab_staging(vr_volume* vol, int mode);
 vr_status vr_get_slab_info(const vr_volume* vol, int h_info[6], float* h_linearize_ms, long long* h_linear_bytes);
 

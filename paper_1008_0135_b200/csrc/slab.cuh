@@ -44,6 +44,36 @@ linearize_kernel(const float* __restrict__ tiled, float* __restrict__ lin, int L
     *reinterpret_cast<float4*>(lin + ((size_t)z * LY + y) * LX + cx * 4) = v;
 }
 
+// Second linear copy for views whose dominant axis is x: float linT[LXT][LY][LZT] with z FASTEST (LZT a multiple of 4),
+// same padded coordinates.  A slab thin along x is then thin along the slowest dimension of its source, as a slab thin
+// along z is for lin[][][].  One CTA transposes a 32(x) x 32(z) patch at one y through shared memory.
+__host__ __device__ inline LinearDims linear_dims_t(int nx, int ny, int nz) {
+    LinearDims L;
+    L.LX = nx + PAD_X + 1;
+    L.LY = ny + PAD_Y + 1;
+    L.LZ = (nz + PAD_Z + 1 + 3) & ~3;
+    return L;
+}
+__global__ void __launch_bounds__(256)
+transpose_kernel(const float* __restrict__ tiled, float* __restrict__ linT, int LX, int LY, int LZ, int z_last,
+                 unsigned ty_stride, unsigned slab_stride) {
+    __shared__ float sm[32][33];
+    const int x0 = blockIdx.x * 32, z0 = blockIdx.z * 32, y = blockIdx.y;
+    const int tx = threadIdx.x & 31, tr = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int zz = tr + 8 * k;
+        const int x = min(x0 + tx, LX - 1), z = min(z0 + zz, z_last);      // z beyond the padded cube: copies of the last layer
+        sm[zz][tx] = __ldg(tiled + tiled_index(x, y, z, ty_stride, slab_stride));
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int xx = tr + 8 * k;
+        if (x0 + xx < LX && z0 + tx < LZ) linT[((size_t)(x0 + xx) * LY + y) * LZ + z0 + tx] = sm[tx][xx];
+    }
+}
+
 #ifndef VR_SLAB_WARP_W
 #define VR_SLAB_WARP_W 16
 #endif
@@ -54,7 +84,8 @@ constexpr int SLAB_MAPS = 4;      // window sizes (tensor maps) a frame may use:
 struct SlabParams {
     int logD;                 // slab thickness D = 1 << logD cell layers along the dominant axis
     int n_maps;               // orthographic: 1; perspective: up to SLAB_MAPS, largest first
-    int w[SLAB_MAPS][3];      // window extent in voxels per axis (dominant axis: D + 1; x: + 3 for the aligned start, a multiple of 4)
+    int w[SLAB_MAPS][3];      // window extent in voxels per axis (dominant axis: D + 1; the source's fastest axis — x, or z for
+                              // x-dominant views — + 3 for the aligned start, a multiple of 4)
     int box_floats[SLAB_MAPS];// w[k][0]*w[k][1]*w[k][2]: what one bulk tensor copy with map k delivers
     int slot_floats;          // floats per buffer: box_floats[0] rounded up to a multiple of 32 (buffers stay 128-byte aligned)
     // The ray of pixel (px,py) in PADDED coordinates, both projections: it passes through Q = q0 + px*dqx + py*dqy with
@@ -96,7 +127,8 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, u
 
 // ------------------------------------------------------------------------------------------------
 // a1 + a3 + a4/a5, slab-staged.  Same grid and CTA shape as cast_kernel (16x8-pixel tiles per brick rectangle).
-// DOM = the dominant axis of the view direction.  Dynamic shared memory: [2 window buffers][256 float4 table]
+// DOM = the dominant axis of the view direction; DOM = x reads the z-fastest copy (window laid out [x][y][z]).
+// Dynamic shared memory: [2 window buffers][256 float4 table]
 // [2 mbarriers][corner rays][origins].
 // ------------------------------------------------------------------------------------------------
 template <int MODE, int DOM>
@@ -171,6 +203,7 @@ cast_slab_kernel(const __grid_constant__ FrameParams P, const __grid_constant__ 
     // Window of a slab on the two other axes: bounding box of the tile's rays between the slab's faces.  U_a(c) is
     // linear-fractional in (px,py) and linear in c, so its extremes over the tile are taken by a corner ray on a face.
     constexpr int A1 = (DOM + 1) % 3, A2 = (DOM + 2) % 3;
+    constexpr int FAST = DOM == 0 ? 2 : 0, SLOW = DOM == 0 ? 0 : 2;       // fastest / slowest axis of the window and its source
     if (tid == 0) {
         const int px0 = br->rx0 + txi * CTA_W, py0 = br->ry0 + tyi * CTA_H;
 #pragma unroll
@@ -203,16 +236,16 @@ cast_slab_kernel(const __grid_constant__ FrameParams P, const __grid_constant__ 
         // fp32 segment arithmetic that places the samples (<= 1e-5 voxel)
         org[A1] = (int)floor(lo1 - SLAB_FUZZ); ext[A1] = (int)floor(hi1 + SLAB_FUZZ) + 2 - org[A1];
         org[A2] = (int)floor(lo2 - SLAB_FUZZ); ext[A2] = (int)floor(hi2 + SLAB_FUZZ) + 2 - org[A2];
-        ext[0] += org[0] & 3;
-        org[0] &= ~3;                                      // the copy must start 16-byte aligned (measured: a start
+        ext[FAST] += org[FAST] & 3;
+        org[FAST] &= ~3;                                   // the copy must start 16-byte aligned (measured: a start
                                                            // coordinate that is not a multiple of 4 floats faults)
         int m = 0;                                         // the smallest window that holds the box (map 0 always does)
         for (int q = 1; q < S.n_maps; ++q)
             if (ext[A1] <= S.w[q][A1] && ext[A2] <= S.w[q][A2]) m = q;
         int* so = s_org + slot * 8;
-        so[0] = org[0]; so[1] = org[1]; so[2] = org[2]; so[3] = S.w[m][0]; so[4] = S.w[m][0] * S.w[m][1];
+        so[0] = org[0]; so[1] = org[1]; so[2] = org[2]; so[3] = S.w[m][FAST]; so[4] = S.w[m][FAST] * S.w[m][1];
         mbar_expect_tx(&bar[slot], (unsigned)S.box_floats[m] * 4u);
-        tma_load_3d(win + (size_t)slot * S.slot_floats, &maps.m[m], &bar[slot], org[0], org[1], org[2]);
+        tma_load_3d(win + (size_t)slot * S.slot_floats, &maps.m[m], &bar[slot], org[FAST], org[1], org[SLOW]);
     };
     if (tid == 0 && ns > 0) issue(0);
 
@@ -227,7 +260,7 @@ cast_slab_kernel(const __grid_constant__ FrameParams P, const __grid_constant__ 
         const int s = s_begin + sgn * k;
         const int w0 = s_org[slot * 8 + 3], w01 = s_org[slot * 8 + 4];
         const float* __restrict__ wbase = win + (size_t)slot * S.slot_floats
-                                          - (s_org[slot * 8 + 0] + s_org[slot * 8 + 1] * w0 + s_org[slot * 8 + 2] * w01);
+                                          - (s_org[slot * 8 + FAST] + s_org[slot * 8 + 1] * w0 + s_org[slot * 8 + SLOW] * w01);
         while (j < n) {
             int jl = j - js;
             if (jl == P.seg_len) {
@@ -237,14 +270,20 @@ cast_slab_kernel(const __grid_constant__ FrameParams P, const __grid_constant__ 
             Cell c;
             locate(An, jl, h, c);
             if (((int)(DOM == 0 ? c.ix : DOM == 1 ? c.iy : c.iz) >> logD) != s) break;
-            const float* __restrict__ p0 = wbase + ((int)c.ix + (int)c.iy * w0 + (int)c.iz * w01);
+            const int i_fast = (int)(DOM == 0 ? c.iz : c.ix), i_slow = (int)(DOM == 0 ? c.ix : c.iz);
+            const float* __restrict__ p0 = wbase + (i_fast + (int)c.iy * w0 + i_slow * w01);
             const float* __restrict__ p1 = p0 + w0;
             const float* __restrict__ p2 = p0 + w01;
             const float* __restrict__ p3 = p2 + w0;
-            const float c00 = fmaf(c.fx, p0[1] - p0[0], p0[0]);
-            const float c10 = fmaf(c.fx, p1[1] - p1[0], p1[0]);
-            const float c01 = fmaf(c.fx, p2[1] - p2[0], p2[0]);
-            const float c11 = fmaf(c.fx, p3[1] - p3[0], p3[0]);
+            // corners v[dz][dy][dx]: the +1 neighbour along the window's fastest axis is the next float
+            const float v000 = p0[0], v010 = p1[0];
+            const float v100 = DOM == 0 ? p0[1] : p2[0], v110 = DOM == 0 ? p1[1] : p3[0];
+            const float v001 = DOM == 0 ? p2[0] : p0[1], v011 = DOM == 0 ? p3[0] : p1[1];
+            const float v101 = DOM == 0 ? p2[1] : p2[1], v111 = p3[1];
+            const float c00 = fmaf(c.fx, v001 - v000, v000);
+            const float c10 = fmaf(c.fx, v011 - v010, v010);
+            const float c01 = fmaf(c.fx, v101 - v100, v100);
+            const float c11 = fmaf(c.fx, v111 - v110, v110);
             const float c0 = fmaf(c.fy, c10 - c00, c00);
             const float c1 = fmaf(c.fy, c11 - c01, c01);
             const float v = fmaf(c.fz, c1 - c0, c0);

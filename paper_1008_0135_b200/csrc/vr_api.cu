@@ -84,9 +84,10 @@ struct vr_volume {
     // slab-staged caster (slab.cuh): linear padded copy, made on first use
     int slab_mode = 1;                // 0 off, 1 auto (dense orthographic frames), 2 whenever the window fits
     int slab_logd = -1;               // env VR_SLAB_LOGD: force the slab thickness (tuning), -1 = heuristic
-    float* d_linear = nullptr;
+    float* d_linear = nullptr;        // x fastest: views whose dominant axis is y or z
+    float* d_linear_t = nullptr;      // z fastest: views whose dominant axis is x
     bool linear_failed = false;       // allocation failed once: stay on the row-cache caster
-    float linearize_ms = 0.f;
+    float linearize_ms = 0.f, transpose_ms = 0.f;
     int last_slab[6] = {0, 0, 0, 0, 0, 0};   // last frame: used, dominant axis, D, window x, y, z
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};   // cast begin/end, composite begin/end
     bool timed_cast = false, timed_comp = false;
@@ -405,7 +406,7 @@ void plan_slab(const vr_volume* vol, const Frame& f, double limit_bytes_per_samp
                             std::fabs(S.dvy[a] * vd - S.dvy[dom] * va) * (vr::CTA_H - 1)) / (vd * vd);
         }
         double wq[3];
-        for (int a = 0; a < 3; ++a) wq[a] = e[a] + (a == 0 ? 5.0 : 2.0);             // the margins of window_scan
+        for (int a = 0; a < 3; ++a) wq[a] = e[a] + (a == (dom == 0 ? 2 : 0) ? 5.0 : 2.0);             // the margins of window_scan
         const double layer = wq[(dom + 1) % 3] * wq[(dom + 2) % 3] * 4.0;            // bytes per cell layer of the window
         const double layers = std::floor(113.0 * 1024.0 / (2.0 * layer));            // what two buffers can hold
         if (layers < 2.0) return;
@@ -419,7 +420,7 @@ void plan_slab(const vr_volume* vol, const Frame& f, double limit_bytes_per_samp
         if (!slab_extents(f, S, dom, D, ext)) return false;
         for (int a = 0; a < 3; ++a) {
             w[a] = a == dom ? D + 1 : (int)std::ceil(ext[a] + 2.0 * vr::SLAB_FUZZ) + 2;   // the kernel's floor(hi + fuzz) + 2 - floor(lo - fuzz)
-            if (a == 0) w[a] = (w[a] + 3 + 3) & ~3;          // + 3: the copy starts at a multiple of 4 voxels
+            if (a == (dom == 0 ? 2 : 0)) w[a] = (w[a] + 3 + 3) & ~3;   // the source's fastest axis: + 3, the copy starts at a multiple of 4 voxels
             if (w[a] > 256) return false;
         }
         return true;
@@ -453,7 +454,8 @@ void plan_slab(const vr_volume* vol, const Frame& f, double limit_bytes_per_samp
         if (k > 0 && k < S.n_maps) {
             S.w[k][a1] = std::max(8, (int)std::ceil(w[a1] * fk));
             S.w[k][a2] = std::max(8, (int)std::ceil(w[a2] * fk));
-            S.w[k][0] = std::min(w[0], (S.w[k][0] + 3) & ~3);
+            const int fa = dom == 0 ? 2 : 0;
+            S.w[k][fa] = std::min(w[fa], (S.w[k][fa] + 3) & ~3);
         }
         S.box_floats[k] = S.w[k][0] * S.w[k][1] * S.w[k][2];
     }
@@ -465,41 +467,53 @@ void plan_slab(const vr_volume* vol, const Frame& f, double limit_bytes_per_samp
     sp.use = true;
 }
 
-vr_status ensure_linear(vr_volume* vol) {
-    if (vol->d_linear) return VR_OK;
-    const vr::LinearDims L = vr::linear_dims(vol->dims[0], vol->dims[1], vol->dims[2]);
-    cudaError_t e = cudaMalloc(&vol->d_linear, (size_t)L.LX * L.LY * L.LZ * sizeof(float));
-    if (e != cudaSuccess) { vol->d_linear = nullptr; vol->linear_failed = true; cudaGetLastError(); return cuda_fail(e, "allocate linear copy"); }
+vr_status ensure_linear(vr_volume* vol, bool transposed) {
+    float*& dst = transposed ? vol->d_linear_t : vol->d_linear;
+    if (dst) return VR_OK;
+    const vr::LinearDims L = transposed ? vr::linear_dims_t(vol->dims[0], vol->dims[1], vol->dims[2])
+                                        : vr::linear_dims(vol->dims[0], vol->dims[1], vol->dims[2]);
+    cudaError_t e = cudaMalloc(&dst, (size_t)L.LX * L.LY * L.LZ * sizeof(float));
+    if (e != cudaSuccess) { dst = nullptr; vol->linear_failed = true; cudaGetLastError(); return cuda_fail(e, "allocate linear copy"); }
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     e = cudaEventCreate(&e0);
     if (e == cudaSuccess) e = cudaEventCreate(&e1);
     if (e == cudaSuccess) e = cudaEventRecord(e0, vol->stream);
     if (e == cudaSuccess) {
-        dim3 grid((L.LX / 4 + 63) / 64, (L.LY + 3) / 4, L.LZ);
-        vr::linearize_kernel<<<grid, 256, 0, vol->stream>>>(vol->d_tiled, vol->d_linear, L.LX, L.LY, L.LZ,
-                                                            ty_stride_of(vol), slab_stride_of(vol));
+        if (transposed) {
+            dim3 grid((L.LX + 31) / 32, L.LY, (L.LZ + 31) / 32);
+            vr::transpose_kernel<<<grid, 256, 0, vol->stream>>>(vol->d_tiled, dst, L.LX, L.LY, L.LZ, vol->dims[2] + vr::PAD_Z,
+                                                                ty_stride_of(vol), slab_stride_of(vol));
+        } else {
+            dim3 grid((L.LX / 4 + 63) / 64, (L.LY + 3) / 4, L.LZ);
+            vr::linearize_kernel<<<grid, 256, 0, vol->stream>>>(vol->d_tiled, dst, L.LX, L.LY, L.LZ, ty_stride_of(vol),
+                                                                slab_stride_of(vol));
+        }
         e = cudaGetLastError();
     }
     if (e == cudaSuccess) e = cudaEventRecord(e1, vol->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(vol->stream);
-    if (e == cudaSuccess) e = cudaEventElapsedTime(&vol->linearize_ms, e0, e1);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(transposed ? &vol->transpose_ms : &vol->linearize_ms, e0, e1);
     if (e0) cudaEventDestroy(e0);
     if (e1) cudaEventDestroy(e1);
-    if (e != cudaSuccess) { cudaFree(vol->d_linear); vol->d_linear = nullptr; vol->linear_failed = true; return cuda_fail(e, "linearize"); }
+    if (e != cudaSuccess) { cudaFree(dst); dst = nullptr; vol->linear_failed = true; return cuda_fail(e, "linearize"); }
     return VR_OK;
 }
 
 vr_status encode_slab_map(vr_volume* vol, SlabPlan& sp) {
     EncodeTiledFn enc = encode_tiled_fn();
     if (!enc) return fail(VR_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
-    const vr::LinearDims L = vr::linear_dims(vol->dims[0], vol->dims[1], vol->dims[2]);
-    const cuuint64_t gdim[3] = {(cuuint64_t)L.LX, (cuuint64_t)L.LY, (cuuint64_t)L.LZ};
-    const cuuint64_t gstr[2] = {(cuuint64_t)L.LX * 4, (cuuint64_t)L.LX * L.LY * 4};
+    const bool tr = sp.dom == 0;                      // x-dominant views read the z-fastest copy: tensor dims (z, y, x)
+    const vr::LinearDims L = tr ? vr::linear_dims_t(vol->dims[0], vol->dims[1], vol->dims[2])
+                                : vr::linear_dims(vol->dims[0], vol->dims[1], vol->dims[2]);
+    const int d0 = tr ? L.LZ : L.LX, d2 = tr ? L.LX : L.LZ;
+    const cuuint64_t gdim[3] = {(cuuint64_t)d0, (cuuint64_t)L.LY, (cuuint64_t)d2};
+    const cuuint64_t gstr[2] = {(cuuint64_t)d0 * 4, (cuuint64_t)d0 * L.LY * 4};
     const cuuint32_t estr[3] = {1, 1, 1};
+    const int fa = tr ? 2 : 0, sl = tr ? 0 : 2;
     for (int k = 0; k < vr::SLAB_MAPS; ++k) {
         const int kk = k < sp.S.n_maps ? k : 0;
-        const cuuint32_t box[3] = {(cuuint32_t)sp.S.w[kk][0], (cuuint32_t)sp.S.w[kk][1], (cuuint32_t)sp.S.w[kk][2]};
-        const CUresult r = enc(&sp.maps.m[k], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, vol->d_linear, gdim, gstr, box, estr,
+        const cuuint32_t box[3] = {(cuuint32_t)sp.S.w[kk][fa], (cuuint32_t)sp.S.w[kk][1], (cuuint32_t)sp.S.w[kk][sl]};
+        const CUresult r = enc(&sp.maps.m[k], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, tr ? vol->d_linear_t : vol->d_linear, gdim, gstr, box, estr,
                                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return fail(VR_ERR_CUDA, "cuTensorMapEncodeTiled failed (code " + std::to_string((int)r) + ")");
@@ -550,14 +564,10 @@ vr_status choose_caster(vr_volume* vol, const Frame& f, int mode, SlabPlan& sp) 
     }
     plan_slab(vol, f, limit, sp);
     if (sp.use && sp.bytes_per_sample > limit) sp.use = false;
-    // Views whose dominant axis is x (the fastest axis in memory): a slab is then a few voxels thick along the rows, the
-    // copy degenerates into hundreds of 32-48-byte rows and the window's bank mapping into 8-way conflicts: measured
-    // 3.3-5.1 ms against 2.3 ms on config 5 (profiles/r02_slab.md).  Such frames stay on the row-cache caster.
-    if (sp.use && vol->slab_mode == 1 && sp.dom == 0) sp.use = false;
     // perspective windows are sized for the far corner of the frame: measured on config 3's cube (profiles/r02_slab.md)
     // they only pay when four CTAs still fit an SM
     if (sp.use && vol->slab_mode == 1 && f.P.proj == VR_PROJ_PERSP && sp.smem > (size_t)56 * 1024) sp.use = false;
-    if (sp.use && ensure_linear(vol) != VR_OK) sp.use = false;            // no memory for the second copy: row-cache caster
+    if (sp.use && ensure_linear(vol, sp.dom == 0) != VR_OK) sp.use = false;            // no memory for the second copy: row-cache caster
     if (sp.use) {
         vr_status s = encode_slab_map(vol, sp);
         if (s != VR_OK) return s;
@@ -708,6 +718,7 @@ void vr_destroy_volume(vr_volume* v) {
     if (v->copy_stream) cudaStreamDestroy(v->copy_stream);
     if (v->d_mask) cudaFree(v->d_mask);
     if (v->d_linear) cudaFree(v->d_linear);
+    if (v->d_linear_t) cudaFree(v->d_linear_t);
     if (v->d_mask_count) cudaFree(v->d_mask_count);
     for (int k = 0; k < 4; ++k)
         if (v->ev[k]) cudaEventDestroy(v->ev[k]);
@@ -1007,10 +1018,11 @@ vr_status vr_set_slab_staging(vr_volume* vol, int mode) {
 vr_status vr_get_slab_info(const vr_volume* vol, int h_info[6], float* h_linearize_ms, long long* h_linear_bytes) {
     if (!vol) return fail(VR_ERR_INVALID_ARG, "vr_get_slab_info: volume is NULL");
     if (h_info) for (int k = 0; k < 6; ++k) h_info[k] = vol->last_slab[k];
-    if (h_linearize_ms) *h_linearize_ms = vol->linearize_ms;
+    if (h_linearize_ms) *h_linearize_ms = vol->linearize_ms + vol->transpose_ms;
     if (h_linear_bytes) {
         const vr::LinearDims L = vr::linear_dims(vol->dims[0], vol->dims[1], vol->dims[2]);
-        *h_linear_bytes = vol->d_linear ? (long long)L.LX * L.LY * L.LZ * 4 : 0;
+        const vr::LinearDims T = vr::linear_dims_t(vol->dims[0], vol->dims[1], vol->dims[2]);
+        *h_linear_bytes = (vol->d_linear ? (long long)L.LX * L.LY * L.LZ * 4 : 0) + (vol->d_linear_t ? (long long)T.LX * T.LY * T.LZ * 4 : 0);
     }
     return VR_OK;
 }
