@@ -253,6 +253,7 @@ def run_ours(args):
     time.sleep(0.3)
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * K)]
     cast_ms, comp_ms = [], []
+    slab_frames = []                                               # per timed frame: rendered by the slab-staged caster?
     barrier()
     t_wall0 = time.time()
     for k in range(K):
@@ -261,6 +262,7 @@ def run_ours(args):
         ev[2 * k].record()
         vol.vr_render(cams[view_of(k)], w.W, w.H, w.step, w.mode, w.ert_alpha, out=out)
         ev[2 * k + 1].record()
+        slab_frames.append(vol.vr_get_slab_info()["used"])         # host-side state, no synchronisation
     barrier()
     t_wall1 = time.time()
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
@@ -311,7 +313,13 @@ def run_ours(args):
 
     # ---- untimed instrumented pass: samples and distinct 32-byte sectors (cube + occupancy mask) per view ----
     used_views = sorted(set(view_of(k) for k in range(K)))
-    meas = {v: vol.vr_measure_units(cams[v], w.W, w.H, w.step, w.mode, w.ert_alpha) for v in used_views}
+    # frames the slab-staged caster rendered evaluate every lattice sample: they are measured with skipping off
+    slab_views = sorted(set(view_of(k) for k in range(K) if slab_frames[k]))
+    meas = {v: vol.vr_measure_units(cams[v], w.W, w.H, w.step, w.mode, w.ert_alpha) for v in used_views if v not in slab_views}
+    if slab_views:
+        vol.vr_set_empty_space_skipping(False)
+        meas.update({v: vol.vr_measure_units(cams[v], w.W, w.H, w.step, w.mode, w.ert_alpha) for v in slab_views})
+        vol.vr_set_empty_space_skipping(not args.no_skip)
     samples = sum(meas[view_of(k)][0][0] for k in range(K))           # lattice samples visited (the oracle's count)
     evaluated = sum(meas[view_of(k)][0][1] for k in range(K))         # of which not passed over by empty-space skipping
     alg_bytes = 32.0 * sum(meas[view_of(k)][1][0] + meas[view_of(k)][1][3] for k in range(K))
@@ -381,7 +389,8 @@ def run_ours(args):
         "gsamples_evaluated_per_s": evaluated / (total_ms * 1e-3) / 1e9 * world,
         "empty_space_skipping": dict(skip_info, dense=dense),
         "stages_ms": {"cast": cast_total_ms / K, "composite": float(sum(comp_ms)) / K},
-        "caster": {"slab_staged_last_frame": vol.vr_get_slab_info()},
+        "caster": {"slab_staged_frames": int(sum(slab_frames)), "row_cache_frames": int(K - sum(slab_frames)),
+                   "slab_info_last_frame": vol.vr_get_slab_info()},
         "relayout": {"ms": relayout_ms, "GBps_read_plus_write": (4.0 * cube.numel() + tiled_bytes) / (relayout_ms * 1e-3) / 1e9
                      if relayout_ms > 0 else None},
         "clocks": clocks,
@@ -392,7 +401,7 @@ def run_ours(args):
                         "frame into pinned host memory, copy of frame k overlapping the casting of frame k+1); latency_value: the "
                         "blocking vr_render_to_host per frame"},
         "gpu_launches": 2 * K if B > 1 or w.mode == 1 else K,          # cast_kernel (+ composite_kernel) per frame
-        "roofline": {"bound": "hbm", "kernel": "cast_kernel<EA>" if w.mode == 0 else "cast_kernel<MIP>",
+        "roofline": {"bound": "hbm", "kernel": ("cast_slab_kernel" if sum(slab_frames) * 2 > K else "cast_kernel") + ("<EA>" if w.mode == 0 else "<MIP>"),
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": alg_bytes / K,
