@@ -39,8 +39,8 @@ UNIT = "ms/frame"
 # `ncu --set full` capture), keyed by the run it was captured on; any other run reports traffic = null.
 NCU_TRAFFIC = {
     # (config, image, mode, bricks, skipping): (bytes per launch, profiles/ file the number comes from)
-    (3, 1024, 0, (2, 2, 2), True): (21.23e9, "profiles/r02_cast_full.md (skipping caster, mean of launches az 10 / 20 deg, read + write)"),
-    (3, 1024, 0, (2, 2, 2), False): (27.20e9, "profiles/r02_cast_full.md (dense caster, mean of launches az 10 / 20 deg, read + write)"),
+    (3, 1024, 0, (2, 2, 2), True): (21.36e9, "profiles/r02_cast_full.md (skipping caster at the final HEAD, mean of launches az 10 / 20 deg, read + write)"),
+    (3, 1024, 0, (2, 2, 2), False): (27.23e9, "profiles/r02_cast_full.md (dense caster at the final HEAD, mean of launches az 10 / 20 deg, read + write)"),
 }
 
 
