@@ -430,7 +430,11 @@ build_mask_kernel(const float* __restrict__ vol, unsigned ty_stride, unsigned sl
     __shared__ unsigned rowbits[8][8];          // [lz][ly]: the 32 cell bits of one cell row
     const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 8, z0 = blockIdx.z * 8;
     const int t = threadIdx.x;
+#ifdef VR_EXP_MORTON
+    const int x_last = (int)(ty_stride >> 15) * 32 - 1;          // last padded x that exists (TX * 8 - 1)
+#else
     const int x_last = (int)(ty_stride >> 9) * 8 - 1;            // last padded x that exists (TX * 8 - 1)
+#endif
     const float thr = x_zero_below - MASK_MARGIN;
     if (t < 81) { (&vis[0][0])[t] = 0ull; (&nanb[0][0])[t] = 0ull; }
     __syncthreads();
