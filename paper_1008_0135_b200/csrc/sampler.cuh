@@ -129,6 +129,22 @@ __device__ __forceinline__ bool cell_occupied(const unsigned long long* __restri
     return (half >> bit) & 1u;
 }
 
+// The 16-byte row-chunk load.  EXPERIMENT -DVR_EXP_L2SIZE=64|128|256: the load's L2 prefetch-size qualifier
+// (ld.global.nc.L2::NNNB) — does asking the L2 for larger fills make the HBM side of the gather more stream-like?
+// (profiles/r02_experiments.md)
+__device__ __forceinline__ float4 load_row_chunk(unsigned long long addr) {
+#ifdef VR_EXP_L2SIZE
+#define VR_STR2(x) #x
+#define VR_STR(x) VR_STR2(x)
+    float4 v;
+    asm volatile("ld.global.nc.L2::" VR_STR(VR_EXP_L2SIZE) "B.v4.f32 {%0, %1, %2, %3}, [%4];"
+                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(addr));
+    return v;
+#else
+    return __ldg(reinterpret_cast<const float4*>(addr));
+#endif
+}
+
 // Trilinear value of the cell (O5) through the row cache.
 // vol_base: address of the tiled cube; ty_stride in elements; slab_bytes = bytes between z-tile slabs.
 __device__ __forceinline__ float sample_cached(unsigned long long vol_base, unsigned ty_stride, unsigned slab_bytes,
@@ -177,7 +193,7 @@ __device__ __forceinline__ float sample_cached(unsigned long long vol_base, unsi
 #pragma unroll
         for (int b = 0; b < 2; ++b) {
             const bool need = xchg || ychg[a] || zchg[b];
-            if (need) K.r[a][b] = __ldg(reinterpret_cast<const float4*>(rp[a][b]));
+            if (need) K.r[a][b] = load_row_chunk(rp[a][b]);
             if (straddle && (need || e_all)) K.e[a][b] = __ldg(reinterpret_cast<const float*>(rp[a][b] + de));
         }
     K.cx = cx; K.hy[0] = wy[0]; K.hy[1] = wy[1]; K.hz[0] = wz[0]; K.hz[1] = wz[1]; K.straddle = straddle;
