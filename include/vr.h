@@ -126,8 +126,9 @@ vr_status vr_get_skip_info(vr_volume* vol, int* h_active, float* h_build_ms, lon
  *     channel mask, frames some of whose rays do not advance along the dominant axis (eye inside the cube, very wide
  *     field of view) and frames whose window does not fit shared memory always use the other caster.
  *     mode 0: never.  mode 1 (default): when the window stages at most ~80 bytes per sample (dense sampling: small pixel
- *     pitch x step), ~130 bytes x the occupied-cell fraction when empty-space skipping is active for the table; for
- *     perspective frames in addition only when four CTAs fit one SM.  mode 2: whenever the window fits.  If the
+ *     pitch x step), ~130 bytes x the occupied-cell fraction when empty-space skipping is active for the table;
+ *     orthographic frames only (perspective windows must hold the far corner tiles; measured, they never paid).
+ *     mode 2: whenever the window fits, perspective frames included.  If the
  *     linear copy cannot be allocated the library stays on the other caster.
  * vr_get_slab_info: h_info[6] = {last frame used the slab caster, dominant axis, slab thickness D in cell layers,
  *     (largest) window extent in voxels along x, y, z}; time spent making the linear copies in ms; their size in bytes

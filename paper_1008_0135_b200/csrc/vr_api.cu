@@ -370,7 +370,7 @@ bool slab_extents(const Frame& f, const vr::SlabParams& S, int dom, int D, doubl
 }
 
 // Decide whether this frame can run on the slab-staged caster and size its windows.
-void plan_slab(const vr_volume* vol, const Frame& f, double limit_bytes_per_sample, SlabPlan& sp) {
+void plan_slab(const vr_volume* vol, const Frame& f, double limit_bytes_per_sample, size_t max_smem, SlabPlan& sp) {
     const vr::FrameParams& P = f.P;
     sp.use = false;
     if (vol->slab_mode == 0 || P.n_runs > 0 || vol->linear_failed || f.total_tiles == 0) return;
@@ -408,7 +408,7 @@ void plan_slab(const vr_volume* vol, const Frame& f, double limit_bytes_per_samp
         double wq[3];
         for (int a = 0; a < 3; ++a) wq[a] = e[a] + (a == (dom == 0 ? 2 : 0) ? 5.0 : 2.0);             // the margins of window_scan
         const double layer = wq[(dom + 1) % 3] * wq[(dom + 2) % 3] * 4.0;            // bytes per cell layer of the window
-        const double layers = std::floor(113.0 * 1024.0 / (2.0 * layer));            // what two buffers can hold
+        const double layers = std::floor((double)max_smem / (2.0 * layer));          // what two buffers can hold
         if (layers < 2.0) return;
         const double Dq = layers >= 9.0 ? 8.0 : layers >= 5.0 ? 4.0 : layers >= 3.0 ? 2.0 : 1.0;
         const double low = layer * (Dq + 1.0) / Dq * std::fabs(P.fwd[dom]) * P.step / (double)vr::CTA_THREADS;
@@ -434,7 +434,7 @@ void plan_slab(const vr_volume* vol, const Frame& f, double limit_bytes_per_samp
     };
     int best = -1, w[3] = {0, 0, 0};
     for (int pass = 0; pass < 2 && best < 0; ++pass) {
-        const size_t budget = pass == 0 ? (size_t)56 * 1024 : (size_t)113 * 1024;   // 4 or 2 CTAs per SM
+        const size_t budget = std::min(max_smem, pass == 0 ? (size_t)56 * 1024 : (size_t)113 * 1024);   // 4 or 2 CTAs per SM
         for (int logd = 3; logd >= 0; --logd) {
             if (vol->slab_logd >= 0 && logd != vol->slab_logd) continue;
             if (!window(logd, w)) continue;
@@ -562,11 +562,12 @@ vr_status choose_caster(vr_volume* vol, const Frame& f, int mode, SlabPlan& sp) 
         const double cells = (double)vol->dims[0] * vol->dims[1] * vol->dims[2];
         limit = skip ? 130.0 * (double)vol->mask_occupied / cells : 80.0;
     }
-    plan_slab(vol, f, limit, sp);
+    // Perspective frames: the windows must hold the far corner tiles and the host has to scan every tile of the frame
+    // for their size (milliseconds at 2048^2); measured on config 3's cube and on config 1 the slab caster never beat
+    // the row-cache caster there (profiles/r02_slab.md).  Automatic choice: orthographic frames only.
+    if (vol->slab_mode == 1 && f.P.proj == VR_PROJ_PERSP) { sp.use = false; vol->last_slab[0] = 0; return VR_OK; }
+    plan_slab(vol, f, limit, (size_t)113 * 1024, sp);
     if (sp.use && sp.bytes_per_sample > limit) sp.use = false;
-    // perspective windows are sized for the far corner of the frame: measured on config 3's cube (profiles/r02_slab.md)
-    // they only pay when four CTAs still fit an SM
-    if (sp.use && vol->slab_mode == 1 && f.P.proj == VR_PROJ_PERSP && sp.smem > (size_t)56 * 1024) sp.use = false;
     if (sp.use && ensure_linear(vol, sp.dom == 0) != VR_OK) sp.use = false;            // no memory for the second copy: row-cache caster
     if (sp.use) {
         vr_status s = encode_slab_map(vol, sp);
