@@ -136,6 +136,19 @@ vr_status vr_get_skip_info(vr_volume* vol, int* h_active, float* h_build_ms, lon
 vr_status vr_set_slab_staging(vr_volume* vol, int mode);
 vr_status vr_get_slab_info(const vr_volume* vol, int h_info[6], float* h_linearize_ms, long long* h_linear_bytes);
 
+/* Host-only planning step of the slab-staged caster, no device needed (what vr_set_slab_staging(vol, 2) would decide
+ *     for this frame): h_plan[8] = {eligible, dominant axis, slab thickness D, window extent x, y, z, window sizes
+ *     in use (1: orthographic), shared memory per CTA in bytes}; *h_bytes_per_sample = window bytes staged per sample.
+ *     h_ray[18] = the affine ray description the kernel's window placement uses, in padded voxel coordinates
+ *     (voxel + (8,1,1) - 1/2): the ray of pixel (px,py) passes through Q = q0 + px*dqx + py*dqy with direction
+ *     V = v0 + px*dvx + py*dvy; order q0[3], dqx[3], dqy[3], v0[3], dvx[3], dvy[3].  Window rule (slab.cuh): for the
+ *     slab of cells [s*D, s*D + D) along the dominant axis the window starts at floor(lo - 1e-3) on the two other
+ *     axes, lo/hi = min/max over the tile's four corner rays and the slab's two faces of
+ *     U_a(c) = Q_a + (c - Q_dom) V_a / V_dom, rounded down to a multiple of 4 on the source's fastest axis (x; z for
+ *     x-dominant views), and must hold voxels up to floor(hi + 1e-3) + 1.                                          */
+vr_status vr_plan_slab(const int dims[3], const int bricks[3], const vr_camera* cam, int W, int H, float step_voxels,
+                       int h_plan[8], double* h_bytes_per_sample, double h_ray[18]);
+
 /* a1-a7  One frame: per-brick ray casting inside each brick's rendering rectangle
  *     (PAPER.md:150), then depth-ordered composition into d_out_rgba.
  *     step_voxels: sampling distance along the ray in voxels, > 0.

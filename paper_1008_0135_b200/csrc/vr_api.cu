@@ -938,6 +938,38 @@ vr_status vr_plan_bricks(const int dims[3], const int bricks[3], const vr_camera
     return VR_OK;
 }
 
+vr_status vr_plan_slab(const int dims[3], const int bricks[3], const vr_camera* cam, int W, int H, float step,
+                       int h_plan[8], double* h_bytes_per_sample, double h_ray[18]) {
+    if (!dims || !bricks || !cam || !h_plan) return fail(VR_ERR_INVALID_ARG, "vr_plan_slab: NULL argument");
+    if (W <= 0 || H <= 0 || W > 32768 || H > 32768) return fail(VR_ERR_INVALID_ARG, "vr_plan_slab: W and H must be in [1,32768]");
+    if (!(step > 0.0f) || !std::isfinite(step)) return fail(VR_ERR_INVALID_ARG, "vr_plan_slab: step_voxels must be positive and finite");
+    for (int a = 0; a < 3; ++a)
+        if (dims[a] <= 0 || dims[a] > 65528 || bricks[a] < 1 || bricks[a] > dims[a])
+            return fail(VR_ERR_INVALID_ARG, "vr_plan_slab: need 0 < dims <= 65528 and 1 <= b_a <= n_a");
+    if ((long long)bricks[0] * bricks[1] * bricks[2] > VR_MAX_BRICKS) return fail(VR_ERR_INVALID_ARG, "vr_plan_slab: more than VR_MAX_BRICKS bricks");
+    if (const char* why = vr::check_camera(*cam)) return fail(VR_ERR_INVALID_ARG, why);
+    vr_volume v;                                   // host fields only: nothing is allocated, nothing touches a device
+    for (int a = 0; a < 3; ++a) { v.dims[a] = dims[a]; v.sub_hi[a] = dims[a]; v.bricks[a] = bricks[a]; }
+    v.TX = (dims[0] + vr::PAD_X + 1 + 7) / 8; v.TY = (dims[1] + vr::PAD_Y + 1 + 7) / 8; v.TZ = (dims[2] + vr::PAD_Z + 1 + 7) / 8;
+    v.slab_mode = 2;
+    Frame f;
+    vr_status s = build_frame(&v, cam, W, H, step, 0.0f, true, false, f);
+    if (s != VR_OK) return s;
+    SlabPlan sp;
+    plan_slab(&v, f, INFINITY, (size_t)113 * 1024, sp);
+    h_plan[0] = sp.use ? 1 : 0;
+    h_plan[1] = sp.use ? sp.dom : 0; h_plan[2] = sp.use ? 1 << sp.S.logD : 0;
+    for (int a = 0; a < 3; ++a) h_plan[3 + a] = sp.use ? sp.S.w[0][a] : 0;
+    h_plan[6] = sp.use ? sp.S.n_maps : 0; h_plan[7] = sp.use ? (int)sp.smem : 0;
+    if (h_bytes_per_sample) *h_bytes_per_sample = sp.use ? sp.bytes_per_sample : 0.0;
+    if (h_ray && sp.use)
+        for (int a = 0; a < 3; ++a) {
+            h_ray[a] = sp.S.q0[a]; h_ray[3 + a] = sp.S.dqx[a]; h_ray[6 + a] = sp.S.dqy[a];
+            h_ray[9 + a] = sp.S.v0[a]; h_ray[12 + a] = sp.S.dvx[a]; h_ray[15 + a] = sp.S.dvy[a];
+        }
+    return VR_OK;
+}
+
 vr_status vr_measure_units(vr_volume* vol, const vr_camera* cam, int W, int H, float step, int mode, float ert,
                            long long h_samples[2], long long h_units[4]) {
     vr_status s = check_render_args(vol, cam, W, H, step, mode);

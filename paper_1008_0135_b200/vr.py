@@ -21,7 +21,7 @@ VR_MAX_CHANNEL_RUNS = 16
 SYMBOLS = ["vr_create_volume", "vr_destroy_volume", "vr_set_stream", "vr_set_transfer_function",
            "vr_set_bricks", "vr_set_subcube", "vr_set_channel_mask", "vr_render", "vr_render_to_host", "vr_render_to_host_async", "vr_wait_frames", "vr_render_bricks", "vr_composite",
            "vr_plan_bricks", "vr_measure", "vr_measure_units", "vr_set_empty_space_skipping", "vr_get_skip_info",
-           "vr_set_l2_fetch_granularity", "vr_set_slab_staging", "vr_get_slab_info",
+           "vr_set_l2_fetch_granularity", "vr_set_slab_staging", "vr_get_slab_info", "vr_plan_slab",
            "vr_get_l2_fetch_granularity", "vr_get_stage_ms", "vr_volume_info", "vr_volume_range", "vr_volume_histogram", "vr_export_linear", "vr_last_error"]
 
 
@@ -73,6 +73,7 @@ def lib():
         L.vr_set_l2_fetch_granularity.argtypes = [C.c_int]
         L.vr_set_slab_staging.argtypes = [vp, C.c_int]
         L.vr_get_slab_info.argtypes = [vp, ip, fp, C.POINTER(C.c_longlong)]
+        L.vr_plan_slab.argtypes = [ip, ip, cam, C.c_int, C.c_int, C.c_float, ip, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.vr_get_l2_fetch_granularity.argtypes = [ip]
         L.vr_get_stage_ms.argtypes = [vp, fp, fp]
         L.vr_volume_info.argtypes = [vp, fp, C.POINTER(C.c_longlong)]
@@ -145,6 +146,18 @@ def vr_plan_bricks(dims, bricks, cam, W, H):
     _check(lib().vr_plan_bricks(_i3(dims), _i3(bricks), C.byref(cam), int(W), int(H),
                                 rect.ctypes.data_as(C.c_void_p), order.ctypes.data_as(C.POINTER(C.c_int))))
     return rect[:B], order[:B]
+
+
+def vr_plan_slab(dims, bricks, cam, W, H, step):
+    """Host-only: what the slab-staged caster would plan for this frame (include/vr.h)."""
+    plan = (C.c_int * 8)()
+    bps = C.c_double(0.0)
+    ray = (C.c_double * 18)()
+    _check(lib().vr_plan_slab(_i3(dims), _i3(bricks), C.byref(cam), int(W), int(H), float(step), plan, C.byref(bps), ray))
+    r = np.array(list(ray), dtype=np.float64).reshape(6, 3)
+    return {"eligible": bool(plan[0]), "dominant_axis": plan[1], "slab_layers": plan[2], "window": (plan[3], plan[4], plan[5]),
+            "n_maps": plan[6], "smem_bytes": plan[7], "bytes_per_sample": bps.value,
+            "q0": r[0], "dqx": r[1], "dqy": r[2], "v0": r[3], "dvx": r[4], "dvy": r[5]}
 
 
 class Volume:

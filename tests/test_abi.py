@@ -65,6 +65,7 @@ def test_null_and_range_checks_without_device(vr):
     assert L.vr_set_l2_fetch_granularity(48) == vr.VR_ERR_INVALID_ARG
     assert L.vr_set_slab_staging(None, 1) == vr.VR_ERR_INVALID_ARG
     assert L.vr_get_slab_info(None, None, None, None) == vr.VR_ERR_INVALID_ARG
+    assert L.vr_plan_slab(None, None, C.byref(cam), 8, 8, 1.0, None, None, None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_get_l2_fetch_granularity(None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_volume_info(None, None, None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_export_linear(None, None) == vr.VR_ERR_INVALID_ARG
