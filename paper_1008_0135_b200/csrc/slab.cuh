@@ -1,16 +1,20 @@
 // slab.cuh — the slab-staged caster (north_star kernel (2): "brick slabs staged through shared memory via TMA
 // where the view is near axis-aligned"; section 2.4).
 //
-// When the rays of a frame are parallel (orthographic) and the pixel pitch times the step is small, many samples
-// fall into every voxel cell and the caster is bound by instruction issue, not by HBM (the ridge at
-// ~14 B per sample).  The row-cache sampler of sampler.cuh spends ~140 of its ~220 instructions per sample on
-// address formation, slot bookkeeping and selects.  Here a CTA instead marches its 16x8-pixel tile through the brick
-// SLAB BY SLAB along the rays' dominant axis: a slab is D cell layers thick; the box of voxels all its rays can touch
-// inside the slab (window, D + 1 layers with the far neighbours) is copied by ONE bulk tensor copy
-// (cp.async.bulk.tensor.3d, SASS UTMALDG) from a LINEAR padded copy of the cube into shared memory, double-buffered
-// with mbarriers, and the eight corners of a sample are eight LDS from one base address plus three adds.
+// When the pixel pitch times the step is small, many samples fall into every voxel cell and the caster is bound by
+// instruction issue, not by HBM (the ridge at ~14 B per sample).  The row-cache sampler of sampler.cuh
+// spends ~140 of its ~220 instructions per sample on address formation, slot bookkeeping and selects.  Here a CTA
+// instead marches its 16x8-pixel tile through the brick SLAB BY SLAB along the dominant axis of the view direction: a
+// slab is D cell layers thick; the box of voxels all its rays can touch inside the slab (window, D + 1 layers with the
+// far neighbours) is copied by ONE bulk tensor copy (cp.async.bulk.tensor.3d, SASS UTMALDG) from a LINEAR padded copy of
+// the cube into shared memory, double-buffered with mbarriers, and the eight corners of a sample are eight LDS from
+// one base address plus three adds.  Orthographic frames: one window size per frame; perspective frames: the window
+// follows the diverging rays (up to four sizes per frame).  Views whose dominant axis is x read a second linear copy
+// with z fastest, so that a slab is always thin along the SLOWEST axis of its source.
 // Positions, cells and fractions come from the same segment-anchored arithmetic as the row-cache caster
 // (sampler.cuh: set_anchor / locate), the lattice, ownership and termination rules are unchanged (O4, O7, O9).
+// Host side (window sizing, choice per frame, tensor maps): vr_api.cu plan_slab / choose_caster; measurements:
+// profiles/r02_slab.md.
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
