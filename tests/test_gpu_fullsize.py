@@ -137,7 +137,7 @@ def test_full_size_ortho_sample_count_law(vr, gass):
 
 # ---- BASELINE.json configs[4]: the sweep's corners at full size (config 3's cube, ORTHO az 30 el 20, ERT off) ----
 @pytest.mark.parametrize("size,step,bricks", [(1024, 0.5, (2, 2, 2)), (1024, 0.25, (2, 2, 2)), (2048, 1.0, (2, 2, 2)),
-                                              (1024, 0.5, (4, 4, 4)), (512, 0.25, (1, 1, 1))])
+                                              (1024, 0.5, (4, 4, 4)), (512, 0.25, (1, 1, 1)), (2048, 0.25, (2, 2, 2))])
 def test_config4_sweep_points_full_size(vr, oracle, gass, size, step, bricks):
     """Step < 1 exercises what step 1 does not: the per-step opacity correction of the table (O6), the hi+lo
     split of the fp32 step vector, several samples per voxel in the row cache (PAPER.md:185 sampling distance;
@@ -148,11 +148,23 @@ def test_config4_sweep_points_full_size(vr, oracle, gass, size, step, bricks):
     px, py = lattice(size, size, stride=size // 128)
     ref = oracle.render_pixels(host, w.table, w.vmin, w.vmax, bricks, oc, size, size, step, 0, 0.0, 0, px, py)["rgba"]
     vol.vr_set_bricks(*bricks)
-    got = vol.vr_render(vr.camera_from_spec(cs), size, size, step, 0, 0.0).cpu().numpy()[py, px]
-    vol.vr_set_bricks(*w.bricks)
     assert ref[:, 3].max() > 0.5
-    report(f"cfg4 EA {size}^2 step {step} bricks {bricks}", got, ref, 1e-4)
-    assert np.abs(got - ref).max() <= 1e-4, np.abs(got - ref).max(axis=0)
+    # both casters at full size: the row-cache caster (slab staging off) and the slab-staged one wherever its window fits
+    used = []
+    for slab_mode in (0, 2, 1):
+        vol.vr_set_slab_staging(slab_mode)
+        got = vol.vr_render(vr.camera_from_spec(cs), size, size, step, 0, 0.0).cpu().numpy()[py, px]
+        info = vol.vr_get_slab_info()
+        used.append(info["used"])
+        if slab_mode == 2 and not info["used"]:
+            continue                                          # window does not fit: same frame as mode 0
+        name = "slab-staged" if info["used"] else "row-cache"
+        report(f"cfg4 EA {size}^2 step {step} bricks {bricks} [{name} caster, staging mode {slab_mode}]", got, ref, 1e-4)
+        assert np.abs(got - ref).max() <= 1e-4, (slab_mode, np.abs(got - ref).max(axis=0))
+    vol.vr_set_bricks(*w.bricks)
+    assert not used[0]
+    if size == 2048:
+        assert used[1] and used[2]                            # the dense points run on the slab caster by default
 
 
 def test_config4_mip_point_oblique_full_size(vr, oracle, gass):
