@@ -265,17 +265,34 @@ cast_slab_kernel(const __grid_constant__ FrameParams P, const __grid_constant__ 
         const int w0 = s_org[slot * 8 + 3], w01 = s_org[slot * 8 + 4];
         const float* __restrict__ wbase = win + (size_t)slot * S.slot_floats
                                           - (s_org[slot * 8 + FAST] + s_org[slot * 8 + 1] * w0 + s_org[slot * 8 + SLOW] * w01);
+        // The segment origin O is folded into the window base, and the slab test runs on the integer part m of the
+        // position relative to O (cell = O + m): cell_dom in [s D, s D + D)  <=>  (unsigned)(m_dom - (s D - O_dom)) < D.
+        const int D = 1 << logD;
+        const float* __restrict__ sbase = wbase + (An.O[FAST] + An.O[1] * w0 + An.O[SLOW] * w01);
+        int lo_m = (s << logD) - An.O[DOM];
         while (j < n) {
             int jl = j - js;
             if (jl == P.seg_len) {
                 js = j; jl = 0;
                 set_anchor(o, d, t_near, P.step, i_lo + js, h, P.seg_span, An);
+                sbase = wbase + (An.O[FAST] + An.O[1] * w0 + An.O[SLOW] * w01);
+                lo_m = (s << logD) - An.O[DOM];
             }
-            Cell c;
-            locate(An, jl, h, c);
-            if (((int)(DOM == 0 ? c.ix : DOM == 1 ? c.iy : c.iz) >> logD) != s) break;
-            const int i_fast = (int)(DOM == 0 ? c.iz : c.ix), i_slow = (int)(DOM == 0 ? c.ix : c.iz);
-            const float* __restrict__ p0 = wbase + (i_fast + (int)c.iy * w0 + i_slow * w01);
+            const float jf = (float)jl;
+            float q[3], r[3];
+            int m[3];
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                q[a] = fmaf(jf, h[a], An.rel[a]);
+                r[a] = __fadd_rd(q[a], 8388608.0f);       // 0 <= q < 2^22: the integer part is the low mantissa bits
+                m[a] = (int)(__float_as_uint(r[a]) & 0x7fffffu);
+            }
+            if ((unsigned)(m[DOM] - lo_m) >= (unsigned)D) break;
+            Cell c;                                        // fractions only: the cell itself is O + m
+            c.fx = q[0] - (r[0] - 8388608.0f);
+            c.fy = q[1] - (r[1] - 8388608.0f);
+            c.fz = q[2] - (r[2] - 8388608.0f);
+            const float* __restrict__ p0 = sbase + (m[FAST] + m[1] * w0 + m[SLOW] * w01);
             const float* __restrict__ p1 = p0 + w0;
             const float* __restrict__ p2 = p0 + w01;
             const float* __restrict__ p3 = p2 + w0;
