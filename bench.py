@@ -40,7 +40,7 @@ UNIT = "ms/frame"
 NCU_TRAFFIC = {
     # (config, image, mode, bricks, skipping): (bytes per launch, profiles/ file the number comes from)
     (3, 1024, 0, (2, 2, 2), True): (21.36e9, "profiles/r02_cast_full.md (skipping caster at the final HEAD, mean of launches az 10 / 20 deg, read + write)"),
-    (5, 1024, 0, (2, 2, 2), True): (5.21e9, "profiles/r02_slab.md (slab-staged caster on config 5, mean of launches az 0 / 10 deg, read + write)"),
+    (5, 1024, 0, (2, 2, 2), True): (5.14e9, "profiles/r02_slab.md (slab-staged caster on config 5, mean of launches az 0 / 10 deg, read + write)"),
     (3, 1024, 0, (2, 2, 2), False): (27.23e9, "profiles/r02_cast_full.md (dense caster at the final HEAD, mean of launches az 10 / 20 deg, read + write)"),
 }
 
