@@ -167,6 +167,29 @@ def test_config4_sweep_points_full_size(vr, oracle, gass, size, step, bricks):
         assert used[1] and used[2]                            # the dense points run on the slab caster by default
 
 
+def test_slab_caster_x_dominant_view_full_size(vr, oracle, gass):
+    """A view whose dominant axis is x (az 100, el 10) at 2048^2, step 1/2: the slab caster reads its z-fastest second
+    copy of the 26.8 GB cube (`transpose_kernel`).  Same lattice and gate as the other config-4 points."""
+    w, cube, host, vol = gass
+    size, step, bricks = 2048, 0.5, (2, 2, 2)
+    cs = wl.orbit_camera(w.dims, 100.0, 10.0, wl.PROJ_ORTHO)
+    oc = oracle.make_camera(cs.view, cs.projection, cs.fovy_deg, cs.ortho_half_h)
+    px, py = lattice(size, size, stride=size // 128)
+    ref = oracle.render_pixels(host, w.table, w.vmin, w.vmax, bricks, oc, size, size, step, 0, 0.0, 0, px, py)["rgba"]
+    assert ref[:, 3].max() > 0.5
+    vol.vr_set_bricks(*bricks)
+    for slab_mode in (0, 2):
+        vol.vr_set_slab_staging(slab_mode)
+        got = vol.vr_render(vr.camera_from_spec(cs), size, size, step, 0, 0.0).cpu().numpy()[py, px]
+        info = vol.vr_get_slab_info()
+        assert info["used"] == (slab_mode == 2) and (slab_mode == 0 or info["dominant_axis"] == 0), info
+        report(f"x-dominant view {size}^2 step {step} [{'slab-staged' if info['used'] else 'row-cache'} caster]", got, ref, 1e-4)
+        assert np.abs(got - ref).max() <= 1e-4
+    print(f"[info] linear copies: {info['linear_bytes'] / 1e9:.2f} GB, made in {info['linearize_ms']:.1f} ms")
+    vol.vr_set_slab_staging(1)
+    vol.vr_set_bricks(*w.bricks)
+
+
 def test_config4_mip_point_oblique_full_size(vr, oracle, gass):
     """The sweep's MIP point (8 bricks, 1024^2, step 1) on the oblique az 30 / el 20 view: raw maxima within
     1e-4 * max(1, |M|) of the oracle's, colours within 1e-4."""
