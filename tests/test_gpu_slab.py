@@ -202,3 +202,37 @@ def test_slab_caster_perspective_eye_inside_or_wide(vr, oracle):
         ref = oracle.render(cube.cpu().numpy(), table, -3.0, 9.0, (2, 2, 2), ocam(oracle, cs), 96, 80, 0.5, 0, 0.0, route=0)["rgba"]
         assert np.abs(got - ref).max() <= TOL_EA, (fov, info)
     vol.close()
+
+
+def test_slab_caster_coarse_steps_and_tiny_images(vr, oracle):
+    """Steps longer than a slab is thick (a ray then has slabs without a sample of its own) and images smaller than one
+    CTA tile."""
+    dims = (90, 64, 77)
+    cube = noisy_cube(dims, 15)
+    table = wl.tf_ramp(0.15)
+    vol = vr.Volume(cube)
+    vol.vr_set_transfer_function(table, -3.0, 9.0)
+    vol.vr_set_bricks(2, 1, 3)
+    for (az, el), (W, H), step in [((30.0, 20.0), (300, 260), 2.5), ((100.0, 10.0), (300, 260), 9.3), ((20.0, 70.0), (11, 5), 0.5),
+                                   ((200.0, -30.0), (1, 1), 0.25)]:
+        cs = wl.orbit_camera(dims, az, el, wl.PROJ_ORTHO)
+        got, _, info = render(vr, vol, cs, W, H, step, 0, 0.0, 2)
+        assert info["used"] == (W > 16), info                 # a few pixels across the cube: the window cannot fit
+        ref = oracle.render(cube.cpu().numpy(), table, -3.0, 9.0, (2, 1, 3), ocam(oracle, cs), W, H, step, 0, 0.0, route=0)["rgba"]
+        assert np.abs(got - ref).max() <= TOL_EA, (az, el, W, H, step, np.abs(got - ref).max())
+    vol.close()
+
+
+def test_slab_caster_image_smaller_than_a_tile(vr, oracle):
+    dims = (9, 7, 8)
+    cube = noisy_cube(dims, 16)
+    table = wl.tf_ramp(0.3)
+    vol = vr.Volume(cube)
+    vol.vr_set_transfer_function(table, -3.0, 9.0)
+    for (W, H) in [(11, 5), (3, 2), (1, 1)]:
+        cs = wl.orbit_camera(dims, 40.0, 25.0, wl.PROJ_ORTHO)
+        got, _, info = render(vr, vol, cs, W, H, 0.25, 0, 0.0, 2)
+        assert info["used"] == (W == 11), info                # windows are sized for a whole 16x8-pixel tile
+        ref = oracle.render(cube.cpu().numpy(), table, -3.0, 9.0, (1, 1, 1), ocam(oracle, cs), W, H, 0.25, 0, 0.0, route=0)["rgba"]
+        assert np.abs(got - ref).max() <= TOL_EA
+    vol.close()
