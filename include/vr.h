@@ -108,6 +108,10 @@ vr_status vr_set_channel_mask(vr_volume* vol, const unsigned char* enabled);
  *     after vr_set_transfer_function changed vmin, vmax or the length of the table's leading run of alpha = 0
  *     (that render synchronises the stream); tables whose second entry already has alpha > 0, and MIP, do not
  *     use it.  Default: enabled.
+ *     MIP frames use the same switch with a different structure: the largest voxel of every block of 4x4x4 cells
+ *     (built once per volume at the first MIP frame, 1/64 of the cube); a sample is passed over when its block's
+ *     maximum is not above the maximum the ray has reached before the current 64-sample segment — a trilinear blend
+ *     never exceeds its corners, so the raw maxima are bit-identical with the switch on and off.
  * vr_get_skip_info: builds the mask if it is due, then reports whether skipping is active for the current table,
  *     the build time of the mask in ms, its size in bytes and the fraction of cells whose bit is set.            */
 vr_status vr_set_empty_space_skipping(vr_volume* vol, int enabled);

@@ -499,6 +499,24 @@ build_mask_kernel(const float* __restrict__ vol, unsigned ty_stride, unsigned sl
     }
 }
 
+// MIP skipping: the largest voxel of every block of 4x4x4 cells (5x5x5 voxels: the cells' far corners included), NaN
+// ignored; same block grid as the occupancy mask.  One thread per block; once per volume, at the first MIP frame.
+__global__ void __launch_bounds__(256)
+build_blockmax_kernel(const float* __restrict__ vol, unsigned ty_stride, unsigned slab_stride, int x_last, int y_last,
+                      int z_last, float* __restrict__ bmax, int NBX, int NBY, int NBZ) {
+    const int bx = blockIdx.x * 64 + (threadIdx.x & 63), by = blockIdx.y * 4 + (threadIdx.x >> 6), bz = blockIdx.z;
+    if (bx >= NBX || by >= NBY || bz >= NBZ) return;
+    float m = -INFINITY;
+    for (int dz = 0; dz < 5; ++dz)
+        for (int dy = 0; dy < 5; ++dy) {
+            const int y = min(by * 4 + dy, y_last), z = min(bz * 4 + dz, z_last);
+#pragma unroll
+            for (int dx = 0; dx < 5; ++dx)
+                m = fmaxf(m, __ldg(vol + tiled_index(min(bx * 4 + dx, x_last), y, z, ty_stride, slab_stride)));
+        }
+    bmax[((size_t)bz * NBY + by) * NBX + bx] = m;
+}
+
 // bits [lo, hi) of a 64-bit set kept as two words, 0 <= lo, hi <= 64
 __device__ __forceinline__ void range_bits(int lo, int hi, unsigned& b_lo, unsigned& b_hi) {
     const unsigned long long m_hi = hi >= 64 ? ~0ull : ((1ull << hi) - 1ull);
@@ -606,6 +624,7 @@ cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ 
             const int je = min(n - js, P.seg_len);
             unsigned en_lo = 0xffffffffu, en_hi = 0xffffffffu;
             if (CHAN) channel_bits(P, o, d, t_near, i_lo + js, je, en_lo, en_hi);
+            const float M_seg = M;                 // MIP skipping decides per segment, with the maximum reached before it
             for (int jl = 0; jl < je; ++jl) {
                 if (CHAN && !(((jl < 32 ? en_lo : en_hi) >> (jl & 31)) & 1u)) continue;   // S2: channel disabled
                 Cell c;
@@ -613,11 +632,15 @@ cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ 
                 ++visited;
                 if (SKIP) {
                     const unsigned tag = (c.iz >> 2) * nbxy + (c.iy >> 2) * nbx + (c.ix >> 2);
-                    if (mask_bitmap) {             // 32-byte sectors of the mask = 4 words
-                        const unsigned sct = tag >> 2, bit = 1u << (sct & 31);
+                    if (mask_bitmap) {             // 32-byte sectors: 4 mask words (EA) or 8 block maxima (MIP)
+                        const unsigned sct = MODE == MODE_EA ? tag >> 2 : tag >> 3, bit = 1u << (sct & 31);
                         if (!(*(volatile unsigned*)(mask_bitmap + (sct >> 5)) & bit)) atomicOr(mask_bitmap + (sct >> 5), bit);
                     }
-                    if (!cell_occupied(mask, nbx, nbxy, c.ix, c.iy, c.iz, mc)) continue;
+                    if (MODE == MODE_EA) {
+                        if (!cell_occupied(mask, nbx, nbxy, c.ix, c.iy, c.iz, mc)) continue;
+                    } else {
+                        if (!(__ldg(reinterpret_cast<const float*>(mask) + tag) > M_seg)) continue;   // cannot raise the maximum
+                    }
                 }
                 Footprint F;
                 fetch_marked(vol, P, c, F, bitmap);
@@ -662,7 +685,30 @@ cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ 
                     channel_bits(P, os, ds, t_near, i_lo + js, je, en_lo, en_hi);
                     todo_lo &= en_lo; todo_hi &= en_hi;
                 }
-                if (SKIP) {                                    // NEXT-2: cells that cannot contribute
+                if (SKIP && MODE == MODE_MIP) {
+                    // MIP: a sample cannot raise the running maximum M when the largest voxel of its 4x4x4-cell block
+                    // (5x5x5 voxels, build_blockmax_kernel) is not above M: a trilinear blend never exceeds its corners.
+                    // Decided per segment with the M reached before it (M only grows, so the test stays valid).
+                    if (have) { M = fmaxf(M, vprev); have = false; }
+                    const float* __restrict__ bmax = reinterpret_cast<const float*>(mask);
+                    unsigned occ_lo = 0u, occ_hi = 0u;
+                    constexpr int G = 8;
+                    for (int jb = 0; jb < je; jb += G) {
+                        float bm[G];
+#pragma unroll
+                        for (int k = 0; k < G; ++k) {
+                            unsigned ix, iy, iz;
+                            locate_cell(An, min(jb + k, je - 1), h, ix, iy, iz);
+                            bm[k] = __ldg(bmax + ((iz >> 2) * nbxy + (iy >> 2) * nbx + (ix >> 2)));
+                        }
+                        unsigned nib = 0u;
+#pragma unroll
+                        for (int k = 0; k < G; ++k) nib |= (bm[k] > M ? 1u : 0u) << k;
+                        if (jb < 32) occ_lo |= nib << jb; else occ_hi |= nib << (jb - 32);
+                    }
+                    todo_lo &= occ_lo; todo_hi &= occ_hi;
+                }
+                if (SKIP && MODE == MODE_EA) {                 // NEXT-2: cells that cannot contribute
                     unsigned occ_lo = 0u, occ_hi = 0u;
                     // VR_OCC_GROUP samples at a time: tags, then the (rare) word loads back to back into registers of
                     // their own, then the bit tests — the loads of a group are in flight together instead of one L2/HBM

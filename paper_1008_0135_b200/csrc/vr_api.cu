@@ -74,6 +74,8 @@ struct vr_volume {
     int seg_max = 64;                 // samples (and voxels of path) per anchored segment; env VR_SEG overrides (1..64)
     bool skip_enabled = true;
     unsigned long long* d_mask = nullptr;
+    float* d_blockmax = nullptr;      // MIP skipping: largest voxel per block of 4x4x4 cells (same grid as the mask words)
+    float blockmax_build_ms = 0.f;
     unsigned long long* d_mask_count = nullptr;
     int NBX = 0, NBY = 0, NBZ = 0;
     size_t mask_words = 0;
@@ -139,6 +141,7 @@ float table_zero_below(const vr_volume* vol) {
 // Empty-space skipping applies to emission-absorption frames whose table starts with at least two transparent
 // entries (otherwise no cell can be proven empty and the mask would be all ones).
 bool skip_applies(const vr_volume* vol, int mode) {
+    if (mode == VR_MODE_MIP) return vol->skip_enabled;        // MIP: blocks whose largest voxel cannot raise the maximum
     return vol->skip_enabled && mode == VR_MODE_EA && table_zero_below(vol) - vr::MASK_MARGIN > 0.0f;
 }
 
@@ -271,21 +274,53 @@ vr_status ensure_mask(vr_volume* vol) {
     return VR_OK;
 }
 
+// MIP skipping: block maxima, once per volume (independent of the table).
+vr_status ensure_blockmax(vr_volume* vol) {
+    if (vol->d_blockmax) return VR_OK;
+    VR_CUDA(cudaMalloc(&vol->d_blockmax, vol->mask_words * sizeof(float)), "allocate block maxima");
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    cudaError_t e = cudaEventCreate(&e0);
+    if (e == cudaSuccess) e = cudaEventCreate(&e1);
+    if (e == cudaSuccess) e = cudaEventRecord(e0, vol->stream);
+    if (e == cudaSuccess) {
+        dim3 grid((vol->NBX + 63) / 64, (vol->NBY + 3) / 4, vol->NBZ);
+        vr::build_blockmax_kernel<<<grid, 256, 0, vol->stream>>>(vol->d_tiled, ty_stride_of(vol), slab_stride_of(vol),
+                                                                 vol->TX * 8 - 1, vol->dims[1] + vr::PAD_Y, vol->dims[2] + vr::PAD_Z,
+                                                                 vol->d_blockmax, vol->NBX, vol->NBY, vol->NBZ);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaEventRecord(e1, vol->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(vol->stream);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&vol->blockmax_build_ms, e0, e1);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (e != cudaSuccess) { cudaFree(vol->d_blockmax); vol->d_blockmax = nullptr; return cuda_fail(e, "build block maxima"); }
+    return VR_OK;
+}
+
+// the per-table (EA) or per-volume (MIP) structure empty-space skipping consults
+vr_status ensure_skip_structure(vr_volume* vol, int mode) {
+    return mode == VR_MODE_MIP ? ensure_blockmax(vol) : ensure_mask(vol);
+}
+
 template <int INSTR>
 vr_status launch_cast(vr_volume* vol, const Frame& f, int mode, float* d_img, unsigned long long* d_counter,
                       unsigned* d_bitmap, unsigned* d_mask_bitmap) {
     if (f.total_tiles == 0) return VR_OK;
     const int B = (int)f.recs.size();
-    const bool skip = skip_applies(vol, mode) && vol->mask_valid;     // callers run ensure_mask first
+    // callers run ensure_skip_structure first
+    const bool skip = skip_applies(vol, mode) && (mode == VR_MODE_MIP ? vol->d_blockmax != nullptr : vol->mask_valid);
+    const unsigned long long* d_skip = mode == VR_MODE_MIP ? reinterpret_cast<const unsigned long long*>(vol->d_blockmax) : vol->d_mask;
 #define VR_LAUNCH(MODE_, SKIP_, CHAN_)                                                                       \
     vr::cast_kernel<MODE_, INSTR, SKIP_, CHAN_><<<f.total_tiles, vr::CTA_THREADS, 0, vol->stream>>>(         \
-        f.P, vol->d_bricks, B, vol->d_tiled, vol->d_tf_ea, vol->d_mask, d_img, d_counter, d_bitmap, d_mask_bitmap)
+        f.P, vol->d_bricks, B, vol->d_tiled, vol->d_tf_ea, d_skip, d_img, d_counter, d_bitmap, d_mask_bitmap)
     const bool chan = f.P.n_runs > 0;
     if (mode == VR_MODE_EA) {
         if (skip) { if (chan) VR_LAUNCH(vr::MODE_EA, 1, 1); else VR_LAUNCH(vr::MODE_EA, 1, 0); }
         else { if (chan) VR_LAUNCH(vr::MODE_EA, 0, 1); else VR_LAUNCH(vr::MODE_EA, 0, 0); }
     } else {
-        if (chan) VR_LAUNCH(vr::MODE_MIP, 0, 1); else VR_LAUNCH(vr::MODE_MIP, 0, 0);
+        if (skip) { if (chan) VR_LAUNCH(vr::MODE_MIP, 1, 1); else VR_LAUNCH(vr::MODE_MIP, 1, 0); }
+        else { if (chan) VR_LAUNCH(vr::MODE_MIP, 0, 1); else VR_LAUNCH(vr::MODE_MIP, 0, 0); }
     }
 #undef VR_LAUNCH
     VR_CUDA(cudaGetLastError(), "cast kernel launch");
@@ -554,13 +589,13 @@ vr_status launch_slab(vr_volume* vol, const Frame& f, const SlabPlan& sp, int mo
 vr_status choose_caster(vr_volume* vol, const Frame& f, int mode, SlabPlan& sp) {
     const bool skip = skip_applies(vol, mode);
     if (skip) {
-        vr_status s = ensure_mask(vol);                                   // builds only after a table change
+        vr_status s = ensure_skip_structure(vol, mode);                   // builds only after a table change (EA) / once (MIP)
         if (s != VR_OK) return s;
     }
     double limit = INFINITY;                                              // mode 2: whenever the window fits
     if (vol->slab_mode == 1) {
         const double cells = (double)vol->dims[0] * vol->dims[1] * vol->dims[2];
-        limit = skip ? 130.0 * (double)vol->mask_occupied / cells : 80.0;
+        limit = !skip ? 80.0 : mode == VR_MODE_MIP ? 20.0 : 130.0 * (double)vol->mask_occupied / cells;
     }
     // Perspective frames: the windows must hold the far corner tiles and the host has to scan every tile of the frame
     // for their size (milliseconds at 2048^2); measured on config 3's cube and on config 1 the slab caster never beat
@@ -718,6 +753,7 @@ void vr_destroy_volume(vr_volume* v) {
     }
     if (v->copy_stream) cudaStreamDestroy(v->copy_stream);
     if (v->d_mask) cudaFree(v->d_mask);
+    if (v->d_blockmax) cudaFree(v->d_blockmax);
     if (v->d_linear) cudaFree(v->d_linear);
     if (v->d_linear_t) cudaFree(v->d_linear_t);
     if (v->d_mask_count) cudaFree(v->d_mask_count);
@@ -979,7 +1015,7 @@ vr_status vr_measure_units(vr_volume* vol, const vr_camera* cam, int W, int H, f
     if ((s = upload_plan(vol, f)) != VR_OK) return s;
     if (mode == VR_MODE_EA && (s = upload_tf_for_step(vol, (double)step)) != VR_OK) return s;
     if ((s = ensure_pool(vol, f.pool_pixels * (mode == VR_MODE_EA ? 4 : 1))) != VR_OK) return s;
-    if (skip_applies(vol, mode) && (s = ensure_mask(vol)) != VR_OK) return s;
+    if (skip_applies(vol, mode) && (s = ensure_skip_structure(vol, mode)) != VR_OK) return s;
     const size_t n_words = (vol->tiled_elems / 8 + 31) / 32;
     const size_t m_words = (vol->mask_words / 4 + 31) / 32 + 1;      // one bit per 32-byte sector (4 words) of the mask
     unsigned *d_bitmap = nullptr, *d_mbitmap = nullptr;

@@ -337,6 +337,7 @@ def test_measure_sector_count_equals_numpy_enumeration(vr, oracle, proj, bricks,
     vol.vr_set_bricks(*bricks)
     (samples, evaluated), units = vol.vr_measure_units(vr.camera_from_spec(cs), W, H, step, 0, 0.0)
     s2, sectors = vol.vr_measure(vr.camera_from_spec(cs), W, H, step, 0, 0.0)
+    vol.vr_set_empty_space_skipping(False)                 # MIP frames would otherwise skip blocks that cannot raise the maximum
     (s3, e3), units_mip = vol.vr_measure_units(vr.camera_from_spec(cs), W, H, step, 1, 0.0)
     vol.close()
     assert evaluated == samples and e3 == s3 and units[3] == 0     # tf_ramp has alpha > 0 from entry 1: no skipping
@@ -469,6 +470,44 @@ def test_empty_space_skipping_leaves_the_frame_bit_identical(vr, oracle, cfg):
         assert ev_on < 0.9 * vis_on and u_on[0] < u_off[0] and u_on[3] > 0 and u_off[3] == 0
         print(f"cfg {cfg} bricks {bricks} step {step}: evaluated {ev_on / vis_on:.3f} of the lattice samples, "
               f"cube sectors {u_on[0] / u_off[0]:.3f} of the unskipped frame")
+    vol.close()
+
+
+@pytest.mark.parametrize("cfg", [2, 3])
+def test_mip_block_maximum_skipping_leaves_the_frame_bit_identical(vr, oracle, cfg):
+    """MIP frames skip the samples of 4x4x4-cell blocks whose largest voxel is not above the maximum the ray has already
+    reached (a trilinear blend never exceeds its corners): raw maxima and colours must be BIT-IDENTICAL with the switch on
+    and off, the oracle gate holds, the lattice count is unchanged and fewer samples are evaluated."""
+    import torch
+    w = wl.config(cfg).scaled(1.0 / 8, W=192, H=160)
+    cube = w.cube("cuda")
+    cube[5:9, 10:20, 30:50] = float("nan")
+    host = cube.cpu().numpy()
+    vol = vr.Volume(cube)
+    vol.vr_set_transfer_function(w.table, w.vmin, w.vmax)
+    vol.vr_set_slab_staging(0)
+    for bricks, proj, step in (((1, 1, 1), wl.PROJ_ORTHO, 1.0), ((2, 2, 2), wl.PROJ_PERSP, 0.5), ((3, 1, 2), wl.PROJ_PERSP, 1.0)):
+        vol.vr_set_bricks(*bricks)
+        cs = wl.orbit_camera(w.dims, 130.0, 20.0, proj)
+        cam = vr.camera_from_spec(cs)
+        res = {}
+        for on in (True, False):
+            vol.vr_set_empty_space_skipping(on)
+            sc = torch.empty((w.H, w.W), dtype=torch.float32, device="cuda")
+            rgba = vol.vr_render(cam, w.W, w.H, step, 1, 0.0, out_scalar=sc).clone()
+            (vis, ev), units = vol.vr_measure_units(cam, w.W, w.H, step, 1, 0.0)
+            torch.cuda.synchronize()
+            res[on] = (rgba, sc.clone(), vis, ev, units)
+        assert torch.equal(res[True][0].view(torch.int32), res[False][0].view(torch.int32))
+        assert torch.equal(res[True][1].view(torch.int32), res[False][1].view(torch.int32))
+        ref = oracle.render(host, w.table, w.vmin, w.vmax, bricks, ocam(oracle, cs), w.W, w.H, step, 1, 0.0, route=1)
+        m, got = ref["scalar"], res[True][1].cpu().numpy()
+        hit = np.isfinite(m)
+        assert (np.isfinite(got) == hit).all()
+        assert (np.abs(got[hit] - m[hit]) <= 1e-4 * np.maximum(1.0, np.abs(m[hit]))).all()
+        assert res[True][2] == res[False][2] == res[False][3] == ref["samples"]
+        assert res[True][3] < 0.95 * res[True][2] and res[True][4][0] < res[False][4][0]   # noise: block maxima sit above most running maxima
+        print(f"cfg {cfg} bricks {bricks} step {step}: MIP evaluates {res[True][3] / res[True][2]:.3f} of the lattice samples")
     vol.close()
 
 
