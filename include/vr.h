@@ -239,6 +239,25 @@ vr_status vr_volume_range(const vr_volume* vol, float* h_min, float* h_max);
  *     counted in the first / last bin, NaN voxels only in *h_nan (may be NULL).  h_counts: HOST, n_bins entries.
  *     One streaming pass over the tiled copy; synchronises.  INVALID_ARG: NULL, n_bins out of range, lo >= hi.     */
 vr_status vr_volume_histogram(vr_volume* vol, int n_bins, float lo, float hi, long long* h_counts, long long* h_nan);
+/* The same histogram for callers that must not allocate device memory: same arguments, same counts, bit for bit.
+ *     Who needs it: (1) an application whose own allocator (PyTorch's caching allocator, an RMM pool) already owns
+ *     nearly all of the GPU — usual once a cube of tens of GB is resident — where a cudaMalloc made behind its back by
+ *     this library fails with "out of memory" although the application has free blocks; (2) a viewer with frames in
+ *     flight on other streams: vr_volume_histogram frees its bins with cudaFree, which waits for the WHOLE device, so
+ *     a histogram asked for while the user drags the data range would stall the frames.  This call makes no
+ *     cudaMalloc / cudaFree and calls nothing that allocates: its bins are a fixed array inside the library image.
+ *     Cost and limit: every GPU that loads libvr_b200.so holds that array — 4097 x 8 = 32 776 bytes — until the
+ *     process ends, whether this call is used or not, and n_bins beyond 4096 is refused (INVALID_ARG, message names
+ *     the limit); the array cannot grow.
+ *     The volume's GPU must be the current device (STATE otherwise): the array exists once per GPU.  The first call
+ *     on each GPU looks up the array's device address (cudaGetSymbolAddress) and remembers it; make that first call
+ *     outside any stream capture.  All calls on one GPU share the array.  Each call clears the part it uses first, so
+ *     what an earlier call left behind does not matter, but two calls that overlap on the GPU (two host threads, two
+ *     volumes on different streams) count into the same bins and both results are garbage: the library takes no
+ *     lock — serialise such calls yourself.  Like vr_volume_histogram it waits for the volume's stream before
+ *     returning.  h_counts: HOST, n_bins entries; h_nan may be NULL.                                              */
+vr_status vr_volume_histogram_noalloc(vr_volume* vol, int n_bins, float lo, float hi, long long* h_counts,
+                                      long long* h_nan);
 /* Inverse of the re-layout: gathers the tiled copy back into d_linear[nz][ny][nx] (round-trip test). */
 vr_status vr_export_linear(vr_volume* vol, float* d_linear);
 

@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1162,3 +1163,85 @@ vr_status vr_export_linear(vr_volume* vol, float* d_linear) {
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// vr_volume_histogram_noalloc — the histogram of vr_volume_histogram for callers that must not allocate.
+//
+// vr_volume_histogram gets its device-side bins from cudaMalloc and gives them back with cudaFree on every call.
+// That is wrong for two kinds of user of this library:
+//   * a viewer embedded in a process whose own allocator (PyTorch's caching allocator, an RMM pool ...) already
+//     holds nearly all of the GPU's memory — normal once a 26.8 GB cube and its copies are resident.  A cudaMalloc
+//     issued from inside this library bypasses that allocator and fails with "out of memory" although the host
+//     application still has free blocks;
+//   * an interaction loop that has frames in flight on other streams: cudaFree waits for the whole device, so a
+//     histogram requested while the user drags the colour-map range would stall every frame being rendered.
+// Here the bins live in the array below, which is part of the library image: every GPU that loads libvr_b200.so
+// holds its (HIST_MAX_BINS + 1) x 8 bytes = 32 776 bytes from then until the process exits, used or not.
+//
+// hist_scratch is a DEVICE symbol.  In host code its name stands for a host-side shadow, not for device memory, so
+// it is never handed to a kernel as it is: the address the kernels get comes from cudaGetSymbolAddress, asked once per
+// device while that device is current (hist_scratch_address).
+// ------------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned long long hist_scratch[vr::HIST_MAX_BINS + 1];   // bins, then the NaN count
+
+namespace {
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+
+// Device address of hist_scratch on the CURRENT device, looked up on the first call per device and remembered.
+vr_status hist_scratch_address(int device, unsigned long long** out) {
+    static std::mutex mtx;
+    static unsigned long long* known[NOALLOC_MAX_DEVICES] = {nullptr};
+    std::lock_guard<std::mutex> lock(mtx);
+    if (device >= 0 && device < NOALLOC_MAX_DEVICES && known[device]) { *out = known[device]; return VR_OK; }
+    void* p = nullptr;
+    VR_CUDA(cudaGetSymbolAddress(&p, hist_scratch), "cudaGetSymbolAddress(histogram scratch)");
+    if (!p) return fail(VR_ERR_CUDA, "vr_volume_histogram_noalloc: the scratch array has no address on this device");
+    if (device >= 0 && device < NOALLOC_MAX_DEVICES) known[device] = static_cast<unsigned long long*>(p);
+    *out = static_cast<unsigned long long*>(p);
+    return VR_OK;
+}
+
+}  // namespace
+
+extern "C" vr_status vr_volume_histogram_noalloc(vr_volume* vol, int n_bins, float lo, float hi, long long* h_counts,
+                                                 long long* h_nan) {
+    if (!vol || !h_counts) return fail(VR_ERR_INVALID_ARG, "vr_volume_histogram_noalloc: NULL argument");
+    if (n_bins < 1) return fail(VR_ERR_INVALID_ARG, "vr_volume_histogram_noalloc: n_bins must be at least 1");
+    if (n_bins > vr::HIST_MAX_BINS)
+        return fail(VR_ERR_INVALID_ARG, "vr_volume_histogram_noalloc: n_bins = " + std::to_string(n_bins) + " exceeds the " +
+                                            std::to_string(vr::HIST_MAX_BINS) +
+                                            " bins the built-in scratch array holds (it cannot grow: this call never allocates)");
+    if (!std::isfinite(lo) || !std::isfinite(hi) || !(hi > lo))
+        return fail(VR_ERR_INVALID_ARG, "vr_volume_histogram_noalloc: need finite lo < hi");
+    // The scratch array exists once per GPU, and the address below is the current device's copy: the volume must live there.
+    int device = -1;
+    VR_CUDA(cudaGetDevice(&device), "cudaGetDevice");
+    cudaPointerAttributes attr;
+    VR_CUDA(cudaPointerGetAttributes(&attr, vol->d_tiled), "cudaPointerGetAttributes(volume)");
+    if (attr.type != cudaMemoryTypeDevice || attr.device != device)
+        return fail(VR_ERR_STATE, "vr_volume_histogram_noalloc: the volume lives on GPU " + std::to_string(attr.device) +
+                                      " but GPU " + std::to_string(device) + " is current (cudaSetDevice to the volume's GPU first)");
+    unsigned long long* d_bins = nullptr;
+    vr_status s = hist_scratch_address(device, &d_bins);
+    if (s != VR_OK) return s;
+    // the array still holds the previous call's counts: bins and NaN counter start from zero
+    VR_CUDA(cudaMemsetAsync(d_bins, 0, (size_t)(n_bins + 1) * sizeof(unsigned long long), vol->stream),
+            "vr_volume_histogram_noalloc: clear scratch");
+    const size_t n_tiles = (size_t)vol->TX * vol->TY * vol->TZ;
+    const float scale = (float)n_bins / (hi - lo);
+    const int grid = (int)std::min<size_t>(n_tiles, 148 * 8);
+    vr::histogram_kernel<<<grid, 256, (size_t)n_bins * sizeof(unsigned), vol->stream>>>(
+        vol->d_tiled, n_tiles, vol->TX, vol->TY, vol->dims[0], vol->dims[1], vol->dims[2], lo, scale, n_bins, d_bins,
+        d_bins + n_bins);
+    VR_CUDA(cudaGetLastError(), "histogram kernel launch");
+    unsigned long long nan = 0;
+    static_assert(sizeof(long long) == sizeof(unsigned long long), "counts are copied as they are");
+    VR_CUDA(cudaMemcpyAsync(h_counts, d_bins, (size_t)n_bins * sizeof(unsigned long long), cudaMemcpyDeviceToHost, vol->stream),
+            "vr_volume_histogram_noalloc: copy bins");
+    VR_CUDA(cudaMemcpyAsync(&nan, d_bins + n_bins, sizeof(nan), cudaMemcpyDeviceToHost, vol->stream),
+            "vr_volume_histogram_noalloc: copy NaN count");
+    VR_CUDA(cudaStreamSynchronize(vol->stream), "vr_volume_histogram_noalloc");
+    if (h_nan) *h_nan = (long long)nan;
+    return VR_OK;
+}

@@ -22,7 +22,7 @@ SYMBOLS = ["vr_create_volume", "vr_destroy_volume", "vr_set_stream", "vr_set_tra
            "vr_set_bricks", "vr_set_subcube", "vr_set_channel_mask", "vr_render", "vr_render_to_host", "vr_render_to_host_async", "vr_wait_frames", "vr_render_bricks", "vr_composite",
            "vr_plan_bricks", "vr_measure", "vr_measure_units", "vr_set_empty_space_skipping", "vr_get_skip_info",
            "vr_set_l2_fetch_granularity", "vr_set_slab_staging", "vr_get_slab_info", "vr_plan_slab",
-           "vr_get_l2_fetch_granularity", "vr_get_stage_ms", "vr_volume_info", "vr_volume_range", "vr_volume_histogram", "vr_export_linear", "vr_last_error"]
+           "vr_get_l2_fetch_granularity", "vr_get_stage_ms", "vr_volume_info", "vr_volume_range", "vr_volume_histogram", "vr_volume_histogram_noalloc", "vr_export_linear", "vr_last_error"]
 
 
 class vr_camera(C.Structure):
@@ -79,6 +79,7 @@ def lib():
         L.vr_volume_info.argtypes = [vp, fp, C.POINTER(C.c_longlong)]
         L.vr_volume_range.argtypes = [vp, fp, fp]
         L.vr_volume_histogram.argtypes = [vp, C.c_int, C.c_float, C.c_float, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
+        L.vr_volume_histogram_noalloc.argtypes = L.vr_volume_histogram.argtypes
         L.vr_export_linear.argtypes = [vp, vp]
         L.vr_last_error.argtypes = []
         L.vr_last_error.restype = C.c_char_p
@@ -314,6 +315,16 @@ class Volume:
         nan = C.c_longlong(0)
         _check(lib().vr_volume_histogram(self._h, int(n_bins), float(lo), float(hi),
                                          counts.ctypes.data_as(C.POINTER(C.c_longlong)), C.byref(nan)))
+        return counts, nan.value
+
+    def vr_volume_histogram_noalloc(self, n_bins, lo, hi):
+        """vr_volume_histogram for callers that must not allocate device memory (a host allocator owns the GPU, or
+        frames are in flight and cudaFree would stall them): same result, bins in a fixed 4096-bin array inside the
+        library.  Calls that overlap on one GPU race; see include/vr.h."""
+        counts = np.zeros(max(int(n_bins), 0), dtype=np.int64)
+        nan = C.c_longlong(0)
+        _check(lib().vr_volume_histogram_noalloc(self._h, int(n_bins), float(lo), float(hi),
+                                                 counts.ctypes.data_as(C.POINTER(C.c_longlong)), C.byref(nan)))
         return counts, nan.value
 
     def vr_export_linear(self):
