@@ -9,8 +9,11 @@ import os
 
 import numpy as np
 
+from . import build as _build
+
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libvr_b200.so")
+# libvr_b200.so; an experiment variant's own file only while VR_DEFINES names that variant (build.py)
+LIB_PATH = _build.lib_path()
 
 VR_OK, VR_ERR_INVALID_ARG, VR_ERR_STATE, VR_ERR_OOM, VR_ERR_CUDA = 0, 1, 2, 3, 4
 VR_MODE_EA, VR_MODE_MIP = 0, 1

@@ -35,6 +35,20 @@ def test_header_symbols_exported(vr):
         assert hasattr(L, n), f"{n} is declared in include/vr.h but not exported"
 
 
+def test_experiment_builds_never_replace_the_product_library(monkeypatch):
+    """A VR_DEFINES build goes to a file of its own, keyed by the defines; every csrc file is a dependency."""
+    monkeypatch.delenv("VR_DEFINES", raising=False)
+    product = vr_build.lib_path()
+    assert product == vr_build.LIB and os.path.basename(product) == "libvr_b200.so"
+    monkeypatch.setenv("VR_DEFINES", "-DVR_EXP_MORTON")
+    a = vr_build.lib_path()
+    monkeypatch.setenv("VR_DEFINES", "-DVR_CTA_H=4 -DVR_CAST_MINBLOCKS=14")
+    b = vr_build.lib_path()
+    assert len({product, a, b}) == 3 and all(p.endswith(".so") for p in (a, b))
+    names = {os.path.basename(p) for p in vr_build.deps()}
+    assert {"vr_api.cu", "kernels.cuh", "sampler.cuh", "slab.cuh", "plan.h", "vr.h"} <= names
+
+
 def test_last_error_never_null(vr):
     assert isinstance(vr.vr_last_error(), str)
 
