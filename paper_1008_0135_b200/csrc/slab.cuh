@@ -188,9 +188,13 @@ cast_slab_kernel(const __grid_constant__ FrameParams P, const __grid_constant__ 
     Anchor An;
     int js = 0;                                            // first sample of the current segment
     if (n > 0) {                                           // slab range of this ray: its first and its last sample
+        // Both with the arithmetic the march below places them with (anchor of the sample's segment + locate): an
+        // anchor of its own at the last sample may disagree with the march by ~5e-6 voxel and, on a slab face, name a
+        // slab the sample is not marched in; that slab would never be staged and the sample dropped.
         Cell c;
-        set_anchor(o, d, t_near, P.step, i_lo + (n - 1), h, P.seg_span, An);
-        locate(An, 0, h, c);
+        const int js_last = ((n - 1) / P.seg_len) * P.seg_len;
+        set_anchor(o, d, t_near, P.step, i_lo + js_last, h, P.seg_span, An);
+        locate(An, (n - 1) - js_last, h, c);
         const int c_last = (int)(DOM == 0 ? c.ix : DOM == 1 ? c.iy : c.iz) >> logD;
         set_anchor(o, d, t_near, P.step, i_lo, h, P.seg_span, An);
         locate(An, 0, h, c);
