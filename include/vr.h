@@ -110,8 +110,9 @@ vr_status vr_set_channel_mask(vr_volume* vol, const unsigned char* enabled);
  *     use it.  Default: enabled.
  *     MIP frames use the same switch with a different structure: the largest voxel of every block of 4x4x4 cells
  *     (built once per volume at the first MIP frame, 1/64 of the cube); a sample is passed over when its block's
- *     maximum is not above the maximum the ray has reached before the current 64-sample segment — a trilinear blend
- *     never exceeds its corners, so the raw maxima are bit-identical with the switch on and off.
+ *     maximum (stored with a margin of 2^-21 of the block's value range and magnitude, which covers what the rounding of
+ *     the fp32 blend can add to its largest corner) is not above the maximum the ray has reached before the current
+ *     64-sample segment, so the raw maxima are bit-identical with the switch on and off.
  * vr_get_skip_info: builds the mask if it is due, then reports whether skipping is active for the current table,
  *     the build time of the mask in ms, its size in bytes and the fraction of cells whose bit is set.            */
 vr_status vr_set_empty_space_skipping(vr_volume* vol, int enabled);

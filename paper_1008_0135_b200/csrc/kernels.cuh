@@ -499,21 +499,31 @@ build_mask_kernel(const float* __restrict__ vol, unsigned ty_stride, unsigned sl
     }
 }
 
-// MIP skipping: the largest voxel of every block of 4x4x4 cells (5x5x5 voxels: the cells' far corners included), NaN
-// ignored; same block grid as the occupancy mask.  One thread per block; once per volume, at the first MIP frame.
+// MIP skipping: an upper bound of every sample value inside a block of 4x4x4 cells (5x5x5 voxels: the cells' far corners
+// included), NaN ignored; same block grid as the occupancy mask.  One thread per block; once per volume, at the first MIP
+// frame.  The bound is the block's largest voxel plus a margin for the rounding of the fp32 blend: a lerp
+// fmaf(w, x - y, y) can pass max(x, y) by the rounding of the difference (<= 2^-24 of the block's value range; at w = 1
+// exactly, which voxel-centred samples of axis-aligned views hit, it returns y + rnd(x - y), not x) and by half an ulp of
+// the result; three nested lerps.  With max + 2^-21 (max - min) + 2^-21 |max| as the stored value a skipped block
+// provably holds no sample above the running maximum, so frames are bit-identical with skipping on and off.
 __global__ void __launch_bounds__(256)
 build_blockmax_kernel(const float* __restrict__ vol, unsigned ty_stride, unsigned slab_stride, int x_last, int y_last,
                       int z_last, float* __restrict__ bmax, int NBX, int NBY, int NBZ) {
     const int bx = blockIdx.x * 64 + (threadIdx.x & 63), by = blockIdx.y * 4 + (threadIdx.x >> 6), bz = blockIdx.z;
     if (bx >= NBX || by >= NBY || bz >= NBZ) return;
-    float m = -INFINITY;
+    float m = -INFINITY, lo = INFINITY;
     for (int dz = 0; dz < 5; ++dz)
         for (int dy = 0; dy < 5; ++dy) {
             const int y = min(by * 4 + dy, y_last), z = min(bz * 4 + dz, z_last);
 #pragma unroll
-            for (int dx = 0; dx < 5; ++dx)
-                m = fmaxf(m, __ldg(vol + tiled_index(min(bx * 4 + dx, x_last), y, z, ty_stride, slab_stride)));
+            for (int dx = 0; dx < 5; ++dx) {
+                const float v = __ldg(vol + tiled_index(min(bx * 4 + dx, x_last), y, z, ty_stride, slab_stride));
+                m = fmaxf(m, v);
+                lo = fminf(lo, v);
+            }
         }
+    if (lo <= m)          // false only when every voxel of the block is NaN (m stays -inf: nothing to find there)
+        m = __fadd_ru(m, __fadd_ru(__fmul_ru(m - lo, 4.76837158203125e-7f), __fmul_ru(fabsf(m), 4.76837158203125e-7f)));
     bmax[((size_t)bz * NBY + by) * NBX + bx] = m;
 }
 
@@ -687,7 +697,7 @@ cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ 
                 }
                 if (SKIP && MODE == MODE_MIP) {
                     // MIP: a sample cannot raise the running maximum M when the largest voxel of its 4x4x4-cell block
-                    // (5x5x5 voxels, build_blockmax_kernel) is not above M: a trilinear blend never exceeds its corners.
+                    // (5x5x5 voxels, build_blockmax_kernel) is not above M (the stored bound covers the rounding of the blend).
                     // Decided per segment with the M reached before it (M only grows, so the test stays valid).
                     if (have) { M = fmaxf(M, vprev); have = false; }
                     const float* __restrict__ bmax = reinterpret_cast<const float*>(mask);

@@ -511,6 +511,46 @@ def test_mip_block_maximum_skipping_leaves_the_frame_bit_identical(vr, oracle, c
     vol.close()
 
 
+def test_mip_skipping_bit_identical_on_voxel_centred_high_dynamic_range_views(vr):
+    """Axis-aligned views with one ray per voxel column and step 1 put every sample on a voxel centre (all three
+    fractions are 0), where the fp32 blend returns y + rnd(x - y) for some corner pairs — a value that can lie a rounding
+    above the larger corner when the two differ by orders of magnitude.  The block maxima carry a margin for that
+    (build_blockmax_kernel): frames must stay bit-identical with skipping on and off, and the maxima equal the
+    column maxima of the cube up to that rounding."""
+    import torch
+    dims = (150, 140, 160)           # rays of more than one 64-sample segment per brick: the test runs from the second on
+    g = torch.Generator(device="cuda").manual_seed(77)
+    mag = 10.0 ** (torch.rand((dims[2], dims[1], dims[0]), generator=g, device="cuda") * 9.0 - 3.0)     # 1e-3 .. 1e6
+    cube = (torch.randn((dims[2], dims[1], dims[0]), generator=g, device="cuda") * mag).contiguous()
+    vol = vr.Volume(cube)
+    vol.vr_set_transfer_function(wl.tf_ramp(0.1), -1.0e6, 1.0e6)
+    vol.vr_set_slab_staging(0)
+    rng = float(cube.max() - cube.min())
+    for axis in range(3):
+        for sign in (1, -1):
+            cs, W, H, ra, rs, ua, us = wl.axis_camera(dims, axis, sign)
+            cam = vr.camera_from_spec(cs)
+            for bricks in ((1, 1, 1), (2, 2, 2)):
+                vol.vr_set_bricks(*bricks)
+                res = {}
+                for on in (True, False):
+                    vol.vr_set_empty_space_skipping(on)
+                    sc = torch.empty((H, W), dtype=torch.float32, device="cuda")
+                    rgba = vol.vr_render(cam, W, H, 1.0, 1, 0.0, out_scalar=sc).clone()
+                    (vis, ev), _ = vol.vr_measure_units(cam, W, H, 1.0, 1, 0.0)
+                    torch.cuda.synchronize()
+                    res[on] = (rgba, sc.clone(), vis, ev)
+                assert torch.equal(res[True][1].view(torch.int32), res[False][1].view(torch.int32)), (axis, sign, bricks)
+                assert torch.equal(res[True][0].view(torch.int32), res[False][0].view(torch.int32)), (axis, sign, bricks)
+                assert res[True][2] == res[False][2] == cube.numel() and res[True][3] < res[False][3]
+                col = cube.amax(dim=2 - axis)                       # [z][y][x] -> maxima along the view axis
+                got = res[True][1]
+                assert got.numel() == col.numel()
+                assert abs(float(got.max()) - float(col.max())) <= 1e-6 * rng
+                assert abs(float(got.sum(dtype=torch.float64)) - float(col.sum(dtype=torch.float64))) <= 1e-6 * rng * col.numel()
+    vol.close()
+
+
 def test_mask_follows_the_transfer_function(vr, oracle):
     """The mask is keyed to the table: after a table change the next frame equals a fresh volume's frame (bit for
     bit) and the oracle's; tables without a transparent leading run and MIP frames do not use the mask."""
