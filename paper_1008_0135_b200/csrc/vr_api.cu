@@ -240,6 +240,11 @@ vr_status upload_tf_for_step(vr_volume* vol, double step) {
     return VR_OK;
 }
 
+// Cells the occupancy mask holds a bit for (and build_mask_kernel counts over): the padded cells, n_a + PAD_a per axis.
+double mask_cells(const vr_volume* vol) {
+    return (double)(vol->dims[0] + vr::PAD_X) * (double)(vol->dims[1] + vr::PAD_Y) * (double)(vol->dims[2] + vr::PAD_Z);
+}
+
 // Build (or reuse) the occupancy mask for the current table.  One pass over the tiled cube.
 vr_status ensure_mask(vr_volume* vol) {
     const float key[3] = {vol->vmin, 1.0f / (vol->vmax - vol->vmin), table_zero_below(vol)};
@@ -559,12 +564,10 @@ vr_status encode_slab_map(vr_volume* vol, SlabPlan& sp) {
 
 template <int MODE, int DOM>
 vr_status launch_slab_t(vr_volume* vol, const Frame& f, const SlabPlan& sp, float* d_img) {
-    static bool attr_set = false;
-    if (!attr_set) {
-        VR_CUDA(cudaFuncSetAttribute(vr::cast_slab_kernel<MODE, DOM>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024),
-                "cudaFuncSetAttribute(slab caster)");
-        attr_set = true;
-    }
+    // the opt-in above 48 KB of dynamic shared memory is a per-device attribute of the function: set on every launch
+    // (a host-side call of about a microsecond) rather than remembered per process, so that volumes on several GPUs work
+    VR_CUDA(cudaFuncSetAttribute(vr::cast_slab_kernel<MODE, DOM>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024),
+            "cudaFuncSetAttribute(slab caster)");
     vr::cast_slab_kernel<MODE, DOM><<<f.total_tiles, vr::CTA_THREADS, sp.smem, vol->stream>>>(
         f.P, sp.S, sp.maps, vol->d_bricks, (int)f.recs.size(), vol->d_tf_ea, d_img);
     VR_CUDA(cudaGetLastError(), "slab caster launch");
@@ -595,8 +598,7 @@ vr_status choose_caster(vr_volume* vol, const Frame& f, int mode, SlabPlan& sp) 
     }
     double limit = INFINITY;                                              // mode 2: whenever the window fits
     if (vol->slab_mode == 1) {
-        const double cells = (double)vol->dims[0] * vol->dims[1] * vol->dims[2];
-        limit = !skip ? 80.0 : mode == VR_MODE_MIP ? 20.0 : 130.0 * (double)vol->mask_occupied / cells;
+        limit = !skip ? 80.0 : mode == VR_MODE_MIP ? 20.0 : 130.0 * (double)vol->mask_occupied / mask_cells(vol);
     }
     // Perspective frames: the windows must hold the far corner tiles and the host has to scan every tile of the frame
     // for their size (milliseconds at 2048^2); measured on config 3's cube and on config 1 the slab caster never beat
@@ -1074,7 +1076,7 @@ vr_status vr_get_skip_info(vr_volume* vol, int* h_active, float* h_build_ms, lon
     if (h_build_ms) *h_build_ms = active ? vol->mask_build_ms : 0.f;
     if (h_mask_bytes) *h_mask_bytes = active ? (long long)(vol->mask_words * sizeof(unsigned long long)) : 0;
     if (h_occupied_fraction)
-        *h_occupied_fraction = active ? (double)vol->mask_occupied / ((double)vol->dims[0] * vol->dims[1] * vol->dims[2]) : 1.0;
+        *h_occupied_fraction = active ? (double)vol->mask_occupied / mask_cells(vol) : 1.0;
     return VR_OK;
 }
 
