@@ -254,6 +254,7 @@ def run_ours(args):
     time.sleep(0.3)
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * K)]
     cast_ms, comp_ms = [], []
+    launches = 0
     slab_frames = []                                               # per timed frame: rendered by the slab-staged caster?
     barrier()
     t_wall0 = time.time()
@@ -278,6 +279,7 @@ def run_ours(args):
         vol.vr_render(cams[view_of(k)], w.W, w.H, w.step, w.mode, w.ert_alpha, out=out)
         c, m = vol.vr_get_stage_ms()
         cast_ms.append(c); comp_ms.append(m)
+        launches += 1 + (1 if m > 0.0 else 0)                     # vr_get_stage_ms reports 0 when no compositor ran
 
     # ---- end to end through the public call with HOST frame buffers (pinned), D2H inside ----
     # e2e: vr_render_to_host_async per frame (plan upload, kernels, D2H of the frame), two host buffers used
@@ -385,9 +387,9 @@ def run_ours(args):
         "frames_per_s_all_gpus": world * K / (total_ms * 1e-3),
         "ms_per_frame_min": min(per_frame), "ms_per_frame_max": max(per_frame),
         "ms_per_view": {str(int(views[view_of(k)])): round(per_frame[k], 3) for k in range(K)},
-        "gsamples_per_s": samples / (total_ms * 1e-3) / 1e9 * world,
-        "samples_per_frame": samples / K, "samples_evaluated_per_frame": evaluated / K,
-        "gsamples_evaluated_per_s": evaluated / (total_ms * 1e-3) / 1e9 * world,
+        "gsamples_evaluated_per_s": evaluated / (total_ms * 1e-3) / 1e9 * world,     # samples interpolated and classified
+        "gsamples_lattice_per_s": samples / (total_ms * 1e-3) / 1e9 * world,         # incl. those empty-space skipping passed over
+        "samples_evaluated_per_frame": evaluated / K, "samples_lattice_per_frame": samples / K,
         "empty_space_skipping": dict(skip_info, dense=dense),
         "stages_ms": {"cast": cast_total_ms / K, "composite": float(sum(comp_ms)) / K},
         "caster": {"slab_staged_frames": int(sum(slab_frames)), "row_cache_frames": int(K - sum(slab_frames)),
@@ -395,13 +397,14 @@ def run_ours(args):
         "relayout": {"ms": relayout_ms, "GBps_read_plus_write": (4.0 * cube.numel() + tiled_bytes) / (relayout_ms * 1e-3) / 1e9
                      if relayout_ms > 0 else None},
         "clocks": clocks,
-        "e2e": {"value": replicas.aggregate_ms_per_frame(e2e_ms, K, world), "unit": UNIT, "h2d_bytes_per_step": B * (72 + 4) + 256,
+        "e2e": {"value": replicas.aggregate_ms_per_frame(e2e_lat_ms, K, world), "unit": UNIT, "h2d_bytes_per_step": B * (72 + 4) + 256,
                 "d2h_bytes_per_step": w.W * w.H * 16,
-                "latency_value": replicas.aggregate_ms_per_frame(e2e_lat_ms, K, world),
-                "note": "value: vr_render_to_host_async per frame + one vr_wait_frames (plan upload + kernels + D2H of the RGBA "
-                        "frame into pinned host memory, copy of frame k overlapping the casting of frame k+1); latency_value: the "
-                        "blocking vr_render_to_host per frame"},
-        "gpu_launches": 2 * K if B > 1 or w.mode == 1 else K,          # cast_kernel (+ composite_kernel) per frame
+                "pipelined_value": replicas.aggregate_ms_per_frame(e2e_ms, K, world),
+                "note": "value: the blocking vr_render_to_host per frame (plan upload + kernels + D2H of the RGBA frame into pinned "
+                        "host memory, each frame fully delivered before the next starts; the round-1 definition); pipelined_value: "
+                        "vr_render_to_host_async per frame + one vr_wait_frames, the copy of frame k overlapping the casting of "
+                        "frame k+1 (what BENCH_r02 reported as value)"},
+        "gpu_launches": launches,          # counted per frame of the stage pass: the caster, + composite_kernel when its events fired
         "roofline": {"bound": "hbm", "kernel": ("cast_slab_kernel" if sum(slab_frames) * 2 > K else "cast_kernel") + ("<EA>" if w.mode == 0 else "<MIP>"),
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
@@ -527,7 +530,8 @@ def run_sweep(args):
         print(json.dumps({"sweep_point": {"mode": "MIP" if mode else "EA", "bricks": B, "step_voxels": step,
                                           "image": f"{size}x{size}", "projection": "perspective45" if args.sweep_persp else "orthographic"},
                           "ms_per_frame_best": best, "ms_per_frame_median": med, "cast_ms_median": cast_med,
-                          "samples": samples, "samples_evaluated": evaluated, "gsamples_per_s": samples / (med * 1e-3) / 1e9,
+                          "samples_evaluated": evaluated, "samples_lattice": samples,
+                          "gsamples_evaluated_per_s": evaluated / (med * 1e-3) / 1e9, "gsamples_lattice_per_s": samples / (med * 1e-3) / 1e9,
                           "algorithmic_GB": 32e-9 * sectors, "bytes_per_sample": 32.0 * sectors / samples,
                           "hbm_GBps_algorithmic": 32e-9 * sectors / (cast_med * 1e-3),
                           "frac_of_peak": 32e-9 * sectors / (cast_med * 1e-3) / peak, "peak": peak,
@@ -535,6 +539,27 @@ def run_sweep(args):
                           "slab": vol.vr_get_slab_info(), "parity": parity}), flush=True)
         del out
     vol.close()
+
+
+def launch_ranks_if_needed(args):
+    """--gpus N must mean N ranks.  Under torchrun (WORLD_SIZE set) the two have to agree; started by hand with N > 1
+    the script re-launches itself as N ranks, one per GPU, the way the driver does (torch.distributed.run on
+    127.0.0.1), and exits with that job's status — it never prints an n_gpus: 1 line for --gpus 8."""
+    world = os.environ.get("WORLD_SIZE")
+    if world is not None:
+        if int(world) != args.gpus:
+            raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}: launch as many ranks as --gpus says")
+        return
+    if args.gpus <= 1 or args.sweep:
+        return
+    import socket
+    import subprocess
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
 
 
 def main():
@@ -558,6 +583,7 @@ def main():
                     help="device-wide L2 fetch granularity hint in bytes (vr_set_l2_fetch_granularity); default: leave as is")
     ap.add_argument("--sweep", action="store_true", help="run BASELINE.json configs[4] (28 points) instead of the headline")
     args = ap.parse_args()
+    launch_ranks_if_needed(args)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.cpu_stride is None:
         args.cpu_stride = 4 if args.impl == "reference" else 1

@@ -55,3 +55,31 @@ def test_two_replicas_render_disjoint_starts_and_time_is_max_over_ranks():
 def test_single_process_is_identity():
     assert replicas.max_over_ranks(3.25, None) == 3.25
     assert [replicas.view_of(k, 0, 1, 36) for k in (0, 35, 36)] == [0, 35, 0]
+
+
+def _run_bench(argv, extra_env):
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    env.update(extra_env)
+    return subprocess.run([sys.executable, os.path.join(root, "bench.py")] + argv, cwd=root, env=env, capture_output=True,
+                          text=True, timeout=600)
+
+
+def test_bench_refuses_a_world_size_that_contradicts_gpus():
+    r = _run_bench(["--gpus", "8", "--steps", "1"], {"WORLD_SIZE": "2", "RANK": "0"})
+    assert r.returncode != 0 and "WORLD_SIZE=2" in r.stderr and "n_gpus" not in r.stdout
+
+
+def test_bench_gpus_n_without_torchrun_launches_n_ranks_itself():
+    """`python bench.py --gpus 2` by hand becomes a 2-rank job (here, without a GPU, both ranks stop with the
+    no-device error): it must never answer with a single-replica line."""
+    if torch.cuda.is_available():
+        import pytest
+        pytest.skip("a GPU is present: the ranks would run the full benchmark")
+    r = _run_bench(["--gpus", "2", "--steps", "1", "--no-cpu-baseline"], {})
+    assert r.returncode != 0
+    assert "n_gpus" not in r.stdout
+    assert "no CUDA device" in r.stderr                  # a rank's own error (the launcher stops the others at the first)
+    assert "torch.distributed" in r.stderr or "elastic" in r.stderr     # ... reported by the multi-rank launcher
