@@ -186,7 +186,80 @@ def test_render_bricks_then_composite_equals_render(vr, oracle):
         else:
             fin = np.isfinite(ref["bricks"])
             assert (np.isfinite(gb) == fin).mean() > 0.999
+            # in value too: a brick's maximum is the oracle's except where a sample within rounding of a shared
+            # face sits in the neighbour's image (A15), which the final frame above is exact about
+            both = fin & np.isfinite(gb)
+            close = np.abs(gb[both] - ref["bricks"][both]) <= 1e-4 * np.maximum(1.0, np.abs(ref["bricks"][both]))
+            assert both.sum() > 1000 and close.mean() > 0.995, close.mean()
+            assert np.abs(vol.vr_render(cam, W, H, 0.5, mode, 0.0).cpu().numpy() - ref["rgba"]).max() <= TOL_EA
         vol.close()
+
+
+def test_samples_on_the_exit_face_and_on_a_brick_plane(vr, oracle):
+    """The dyadic tie cases of tests/test_oracle_edges.py through the C ABI (O4, O9): image plane inside the
+    cube at z = 1, step 2, rays along +z -> samples at z = 2, 4, 6; z = 8 lies exactly on the exit face (not taken) and
+    z = 4 exactly on the plane between the bricks of a (1,1,2) partition (owned by the brick behind the plane).  The
+    geometry is exact in fp32 and fp64, so here the brick images must match the oracle's too, not only the frame."""
+    import torch
+    dims = (4, 4, 8)
+    g = np.random.default_rng(5)
+    host = (g.normal(size=(8, 4, 4)) * 1.5 + 2.0).astype(np.float32)
+    cube = torch.from_numpy(host).cuda()
+    table = wl.tf_ramp(0.3)
+    cs = wl.CameraSpec(wl.look_at((2.0, 2.0, 1.0), (2.0, 2.0, 5.0)), wl.PROJ_ORTHO, 45.0, 2.0)
+    W = H = 4
+    cam = vr.camera_from_spec(cs)
+    vol = vr.Volume(cube)
+    vol.vr_set_transfer_function(table, -3.0, 8.0)
+    for slab_mode in (0, 2):
+        vol.vr_set_slab_staging(slab_mode)
+        for bricks in ((1, 1, 1), (1, 1, 2)):
+            vol.vr_set_bricks(*bricks)
+            ref = oracle.render(host, table, -3.0, 8.0, bricks, ocam(oracle, cs), W, H, 2.0, 0, 0.0, route=1, want_bricks=True)
+            assert ref["samples"] == 3 * W * H
+            got = vol.vr_render(cam, W, H, 2.0, 0, 0.0)
+            imgs = vol.vr_render_bricks(cam, W, H, 2.0, 0, 0.0)
+            torch.cuda.synchronize()
+            assert np.abs(got.cpu().numpy() - ref["rgba"]).max() <= TOL_EA
+            assert np.abs(imgs.cpu().numpy() - ref["bricks"]).max() <= TOL_EA, (slab_mode, bricks)
+            assert vol.vr_measure(cam, W, H, 2.0, 0, 0.0)[0] == ref["samples"]          # bit-exact lattice count
+    # MIP: layer 7 holds the largest values and is only reachable through the sample on the exit face
+    ramp = np.zeros((8, 4, 4), dtype=np.float32)
+    for k in range(8):
+        ramp[k] = float(k)
+    ramp[7] = 100.0
+    vol2 = vr.Volume(torch.from_numpy(ramp).cuda())
+    vol2.vr_set_transfer_function(wl.tf_ramp(0.1), 0.0, 100.0)
+    for slab_mode in (0, 2):
+        vol2.vr_set_slab_staging(slab_mode)
+        sc = torch.empty((H, W), dtype=torch.float32, device="cuda")
+        vol2.vr_render(cam, W, H, 2.0, 1, 0.0, out_scalar=sc)
+        torch.cuda.synchronize()
+        assert torch.equal(sc, torch.full((H, W), 5.5, device="cuda"))
+    vol.close()
+    vol2.close()
+
+
+def test_top_interval_of_the_table(vr, oracle):
+    """O6's last interval through the C ABI: a table that is curved over entries 253..255 (tests/test_oracle_edges.py);
+    cubes of constant value at table positions 253.5, 254.5 and 255 -> A = 1 - (1 - a)^4, C = A * colour."""
+    import torch
+    tab = wl.tf_ramp(0.05).astype(np.float64)
+    tab[253] = (0.9, 0.1, 0.2, 0.1); tab[254] = (0.2, 0.8, 0.3, 0.2); tab[255] = (0.1, 0.3, 0.7, 0.9)
+    tab = tab.astype(np.float32)
+    cs, W, H, *_ = wl.axis_camera((4, 4, 4), 2, 1)
+    cam = vr.camera_from_spec(cs)
+    for x in (253.5, 254.5, 255.0, 300.0):
+        cube = torch.full((4, 4, 4), x, device="cuda")
+        vol = vr.Volume(cube)
+        vol.vr_set_transfer_function(tab, 0.0, 255.0)
+        got = vol.vr_render(cam, W, H, 1.0, 0, 0.0).cpu().numpy()
+        vol.close()
+        e = np.array([np.interp(min(x, 255.0), np.arange(256.0), tab[:, c].astype(np.float64)) for c in range(4)])
+        A = 1.0 - (1.0 - e[3]) ** 4
+        assert np.abs(got[..., 3] - A).max() <= TOL_EA and np.abs(got[..., :3] - A * e[:3]).max() <= TOL_EA, x
+        ref = oracle.render(cube.cpu().numpy(), tab, 0.0, 255.0, (1, 1, 1), ocam(oracle, cs), W, H, 1.0, 0, 0.0, route=0)["rgba"]
+        assert np.abs(got - ref).max() <= TOL_EA
 
 
 def test_nan_block_is_skipped(vr, oracle):
