@@ -15,6 +15,9 @@
  * calls return without synchronising unless stated.  Every call returns a vr_status; the message
  * for the last failure on the calling thread is vr_last_error().  Nothing throws or aborts.
  * There is NO CPU fallback: without a CUDA device every compute call returns VR_ERR_CUDA.
+ * Environment: one variable, read at vr_create_volume.  VR_DEBUG=1 makes every frame call wait for each of its
+ * kernels (caster, compositor) and return that kernel's failure, instead of letting an asynchronous fault surface at
+ * a later call; for debugging only, it serialises the stream.  Nothing else is read from the environment.
  *
  * Geometry conventions (O1-O3, O11):
  *   cube       float32, dims (nx,ny,nz), x fastest: data[(z*ny + y)*nx + x]; voxel (i,j,k) is the
@@ -199,36 +202,6 @@ vr_status vr_composite(vr_volume* vol, const vr_camera* cam, int W, int H, int m
 vr_status vr_plan_bricks(const int dims[3], const int bricks[3], const vr_camera* cam, int W, int H,
                          int out_rect[][4], int out_order[]);
 
-/* Measurement aids (not on the product path):
- * vr_measure: renders the frame with the instrumented build of the caster and returns, in HOST
- *     counters, the lattice samples visited (every sample of O4 up to early termination: the oracle's
- *     count) and the number of distinct 32-byte sectors of the tiled cube that the evaluated samples'
- *     2x2x2 footprints touched (algorithmic HBM bytes of the cube = 32 * that).
- *     Synchronises.  Either output may be NULL.                                                  */
-vr_status vr_measure(vr_volume* vol, const vr_camera* cam, int W, int H, float step_voxels, int mode,
-                     float ert_alpha, long long* h_samples, long long* h_sectors);
-/* vr_measure_units: the full set of counters of the instrumented caster (which takes the same skip and termination
- *     decisions as the product caster).  h_samples[0] = lattice samples visited (= vr_measure's, the oracle's
- *     count), h_samples[1] = samples evaluated (visited minus those empty-space skipping passed over).
- *     h_units[0..2] = distinct 32-byte sectors (= vr_measure's), 64-byte sector pairs and 128-byte lines of the
- *     tiled cube that the EVALUATED samples' footprints touched — what a memory system fetching 32, 64 or 128
- *     bytes per miss has to move; h_units[3] = distinct 32-byte sectors of the occupancy mask that were read.
- *     Either array may be NULL.                                                                                 */
-vr_status vr_measure_units(vr_volume* vol, const vr_camera* cam, int W, int H, float step_voxels, int mode,
-                           float ert_alpha, long long h_samples[2], long long h_units[4]);
-/* Device-wide hint for the number of bytes the L2 fetches from HBM per miss (cudaLimitMaxL2FetchGranularity):
- *     32, 64 or 128.  The caster touches 32-byte sectors sparsely where rays are further apart than a voxel
- *     (the step guarantees every voxel a ray intersects is sampled, not every voxel of the cube), so
- *     the granularity decides how much untouched data rides along.  Affects the whole device (all volumes, all
- *     other kernels of the process).  vr_get_... reads the current value.  INVALID_ARG for any other size.       */
-vr_status vr_set_l2_fetch_granularity(int bytes);
-vr_status vr_get_l2_fetch_granularity(int* h_bytes);
-/* Device time, in ms, of the cast kernel and of the composite kernel of the most recent vr_render /
- *     vr_render_to_host on this volume (CUDA events recorded on the volume's stream around each
- *     launch; composite is 0 when a single brick wrote the frame directly).  Waits for that frame. */
-vr_status vr_get_stage_ms(vr_volume* vol, float* h_cast_ms, float* h_composite_ms);
-/* Device time of the re-layout kernel of vr_create_volume, in ms, and the bytes it allocated.  */
-vr_status vr_volume_info(const vr_volume* vol, float* h_relayout_ms, long long* h_tiled_bytes);
 /* Minimum and maximum of the cube (NaN voxels ignored), computed by the re-layout pass of vr_create_volume at
  *     no extra memory traffic: the data range a transfer function is set over when the file metadata does not
  *     give one ("each GPU computes the minimum and maximum of its portion").
@@ -259,9 +232,6 @@ vr_status vr_volume_histogram(vr_volume* vol, int n_bins, float lo, float hi, lo
  *     returning.  h_counts: HOST, n_bins entries; h_nan may be NULL.                                              */
 vr_status vr_volume_histogram_noalloc(vr_volume* vol, int n_bins, float lo, float hi, long long* h_counts,
                                       long long* h_nan);
-/* Inverse of the re-layout: gathers the tiled copy back into d_linear[nz][ny][nx] (round-trip test). */
-vr_status vr_export_linear(vr_volume* vol, float* d_linear);
-
 const char* vr_last_error(void); /* thread-local, never NULL */
 
 #ifdef __cplusplus

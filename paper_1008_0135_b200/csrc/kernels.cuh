@@ -57,7 +57,6 @@ struct FrameParams {
     int ert_on;
     int seg_len, seg_span;                    // samples per anchored segment; ceil(seg_len*step)+1 (sampler.cuh)
     int nbx, nby;                             // occupancy-mask words (4^3 cells) per row / per column
-    int pf_every, pf_ahead;                   // VR_EXP_L2PREFETCH builds only (env VR_PF), else 0
     int n_runs;                               // S2 channel mask: runs of enabled channels (0 = no mask)
     int run_z[2 * MAX_RUNS];                  // [za, zb) per run, ascending
 };
@@ -71,30 +70,12 @@ struct BrickRec {
     int pad;
 };
 
-// Tile order.  Product build: tiles in plain row-major order, tile (tx,ty,tz) at ((tz*TY + ty)*TX + tx).
-// EXPERIMENT -DVR_EXP_MORTON (north_star kernel (1): "Morton-ordered ... tiled layout"; measured and rejected,
-// profiles/r02_experiments.md): macro-blocks of 4x4x4 tiles (32^3 voxels, 128 KB) in row-major order, the 64 tiles of
-// a macro-block in Morton (Z) order: tile-index bits z1 y1 x1 z0 y0 x0.  The address stays separable,
-// off = fx(x) + fy(y) + fz(z); "ty_stride" / "slab_stride" then are the element strides between macro-blocks
-// adjacent in y / z (TX/4 * 32768, TX/4 * TY/4 * 32768) and TX, TY, TZ are multiples of 4.
-#ifdef VR_EXP_MORTON
-__host__ __device__ __forceinline__ unsigned tile_fx(unsigned x) {              // element offset contributed by padded x
-    const unsigned t = x >> 3;
-    return ((t & ~3u) << 13) | ((t & 2u) << 11) | ((t & 1u) << 9) | (x & 7u);
-}
-__host__ __device__ __forceinline__ unsigned tile_fy(unsigned y, unsigned ty_stride) {
-    const unsigned t = y >> 3;
-    return (t >> 2) * ty_stride + (((t & 2u) << 12) | ((t & 1u) << 10) | ((y & 7u) << 3));
-}
-__host__ __device__ __forceinline__ size_t tile_fz(unsigned z, unsigned slab_stride) {
-    const unsigned t = z >> 3;
-    return (size_t)(t >> 2) * slab_stride + (((t & 2u) << 13) | ((t & 1u) << 11) | ((z & 7u) << 6));
-}
-#else
+// Tile order: plain row-major, tile (tx,ty,tz) at ((tz*TY + ty)*TX + tx); the address is separable,
+// off = fx(x) + fy(y) + fz(z).  (north_star kernel (1) also names a Morton order of the tiles: measured in round 2 as a
+// build switch and rejected, +6-7 % frame time; profiles/r02_experiments.md names the commit that still carries it.)
 __host__ __device__ __forceinline__ unsigned tile_fx(unsigned x) { return (x >> 3) * TILE_ELEMS + (x & 7u); }
 __host__ __device__ __forceinline__ unsigned tile_fy(unsigned y, unsigned ty_stride) { return (y >> 3) * ty_stride + ((y & 7u) << 3); }
 __host__ __device__ __forceinline__ size_t tile_fz(unsigned z, unsigned slab_stride) { return (size_t)(z >> 3) * slab_stride + ((z & 7u) << 6); }
-#endif
 
 // ------------------------------------------------------------------------------------------------
 // a0  re-layout.  The tiled copy holds the cube in PADDED coordinates u = voxel index + PAD_a (8, 1, 1): replicated
@@ -166,12 +147,7 @@ relayout_kernel(const float* __restrict__ src, float* __restrict__ dst, int nx, 
         }
     }
     const int ntile = min(8, TX - tx0);
-#ifdef VR_EXP_MORTON
-    const unsigned ys = (unsigned)(TX >> 2) * 32768u, zs = ys * (unsigned)(TY >> 2);
-    float* const out_yz = dst + tile_fz((unsigned)tz * 8u, zs) + tile_fy((unsigned)ty * 8u, ys);
-#else
     float4* out = reinterpret_cast<float4*>(dst + ((size_t)((size_t)tz * TY + ty) * TX + tx0) * TILE_ELEMS);
-#endif
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
         const int j = t + 256 * k;           // float4 index inside the 8-tile run
@@ -179,11 +155,7 @@ relayout_kernel(const float* __restrict__ src, float* __restrict__ dst, int nx, 
         if (tile < ntile) {
             const int row = r >> 1, lxq = r & 1;
             const float4 v = *reinterpret_cast<const float4*>(&sm[row][tile * 8 + lxq * 4]);
-#ifdef VR_EXP_MORTON
-            reinterpret_cast<float4*>(out_yz + tile_fx((unsigned)(tx0 + tile) * 8u))[r] = v;
-#else
             out[j] = v;
-#endif
         }
     }
 }
@@ -205,16 +177,7 @@ histogram_kernel(const float* __restrict__ tiled, size_t n_tiles, int TX, int TY
     __syncthreads();
     unsigned nans = 0;
     for (size_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-#ifdef VR_EXP_MORTON
-        const size_t mb = tile >> 6;
-        const unsigned rr = (unsigned)(tile & 63);
-        const int MX = TX >> 2, MY = TY >> 2;
-        const int tx = (int)(mb % MX) * 4 + (int)((rr & 1u) | ((rr >> 2) & 2u));
-        const int ty = (int)((mb / MX) % MY) * 4 + (int)(((rr >> 1) & 1u) | ((rr >> 3) & 2u));
-        const int tz = (int)(mb / ((size_t)MX * MY)) * 4 + (int)(((rr >> 2) & 1u) | ((rr >> 4) & 2u));
-#else
         const int tx = (int)(tile % TX), ty = (int)((tile / TX) % TY), tz = (int)(tile / ((size_t)TX * TY));
-#endif
         const float4* src = reinterpret_cast<const float4*>(tiled + tile * TILE_ELEMS);
         for (int q = threadIdx.x; q < TILE_ELEMS / 4; q += 256) {
             const float4 v4 = __ldcs(src + q);
@@ -430,11 +393,7 @@ build_mask_kernel(const float* __restrict__ vol, unsigned ty_stride, unsigned sl
     __shared__ unsigned rowbits[8][8];          // [lz][ly]: the 32 cell bits of one cell row
     const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 8, z0 = blockIdx.z * 8;
     const int t = threadIdx.x;
-#ifdef VR_EXP_MORTON
-    const int x_last = (int)(ty_stride >> 15) * 32 - 1;          // last padded x that exists (TX * 8 - 1)
-#else
     const int x_last = (int)(ty_stride >> 9) * 8 - 1;            // last padded x that exists (TX * 8 - 1)
-#endif
     const float thr = x_zero_below - MASK_MARGIN;
     if (t < 81) { (&vis[0][0])[t] = 0ull; (&nanb[0][0])[t] = 0ull; }
     __syncthreads();
@@ -674,9 +633,6 @@ cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ 
         const unsigned slab_bytes = P.slab_stride * 4u;
         float vprev = 0.f;
         bool have = false, done = false;
-#ifdef VR_EXP_L2PREFETCH
-        unsigned pf_last = 0xffffffffu;
-#endif
         for (int js = 0; js < n && !done; js += P.seg_len) {
             // In the two-pass variants the ray is re-derived from the pixel here (same expressions, same doubles)
             // rather than kept: twelve live double registers across both passes spilled to local memory (measured:
@@ -777,26 +733,6 @@ cast_kernel(const __grid_constant__ FrameParams P, const BrickRec* __restrict__ 
                 }
             } else {
                 for (int jl = 0; jl < je; ++jl) {
-#ifdef VR_EXP_L2PREFETCH
-                    // EXPERIMENT, rejected (profiles/r02_experiments.md).  Build: VR_DEFINES=-DVR_EXP_L2PREFETCH
-                    // python -m paper_1008_0135_b200.build; run with VR_PF=every,ahead.  Every `every` samples the ray
-                    // looks `ahead` samples on and, when that point lies in an 8^3 tile it has not asked for yet, has
-                    // the bulk-copy engine pull the whole 2 KB tile into the L2 (cp.async.bulk.prefetch.L2, SASS UBLKPF);
-                    // lanes that want the same tile are merged with match.any.
-                    if (P.pf_every && ((unsigned)(js + jl) & (unsigned)(P.pf_every - 1)) == 0u && js + jl + P.pf_ahead < n) {
-                        unsigned ax, ay, az;
-                        locate_cell(An, jl + P.pf_ahead, h, ax, ay, az);
-                        const unsigned tid = (az >> 3) * (P.slab_stride >> 9) + (ay >> 3) * (P.ty_stride >> 9) + (ax >> 3);
-                        if (tid != pf_last) {
-                            pf_last = tid;
-                            const unsigned peers = __match_any_sync(__activemask(), tid);
-                            if ((peers & ((1u << (threadIdx.x & 31)) - 1u)) == 0u) {
-                                const unsigned long long a = vol_base + (unsigned long long)tid * (TILE_ELEMS * 4ull);
-                                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(a), "r"(TILE_ELEMS * 4) : "memory");
-                            }
-                        }
-                    }
-#endif
                     Cell c;
                     locate(An, jl, h, c);
                     const float v = sample_cached(vol_base, P.ty_stride, slab_bytes, c, K);

@@ -9,7 +9,7 @@
 // split into an integer origin O and a remainder rel in [0, seg span], and inside the segment
 // q_rel(j') = rel + j' h in fp32 with |q_rel| <= ~65: rounding <= 4e-6 voxel.  Voxel index = O + floor(q_rel).
 //
-// Row cache.  ncu of the first caster (profiles/r01cd_cast_full.md) showed the L1TEX data stage at 96 %: eight
+// Row cache.  ncu of the round-1 caster showed the L1TEX data stage at 96 %: eight
 // scalar corner loads per sample, each a warp request over ~20-32 distinct lines.  Here a ray keeps, in
 // registers, the four 16-byte x-chunks (4 voxels each) that hold its current 2x2 (y,z) rows and loads a
 // row only when the ray has moved off it:
@@ -129,20 +129,10 @@ __device__ __forceinline__ bool cell_occupied(const unsigned long long* __restri
     return (half >> bit) & 1u;
 }
 
-// The 16-byte row-chunk load.  EXPERIMENT -DVR_EXP_L2SIZE=64|128|256: the load's L2 prefetch-size qualifier
-// (ld.global.nc.L2::NNNB) — does asking the L2 for larger fills make the HBM side of the gather more stream-like?
-// (profiles/r02_experiments.md)
+// The 16-byte row-chunk load (read-only path).  Larger L2 fill sizes (ld.global.nc.L2::NNNB) were measured in round 2:
+// no gain (profiles/r02_experiments.md).
 __device__ __forceinline__ float4 load_row_chunk(unsigned long long addr) {
-#ifdef VR_EXP_L2SIZE
-#define VR_STR2(x) #x
-#define VR_STR(x) VR_STR2(x)
-    float4 v;
-    asm volatile("ld.global.nc.L2::" VR_STR(VR_EXP_L2SIZE) "B.v4.f32 {%0, %1, %2, %3}, [%4];"
-                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(addr));
-    return v;
-#else
     return __ldg(reinterpret_cast<const float4*>(addr));
-#endif
 }
 
 // Trilinear value of the cell (O5) through the row cache.
@@ -169,25 +159,15 @@ __device__ __forceinline__ float sample_cached(unsigned long long vol_base, unsi
 #pragma unroll
     for (int b = 0; b < 2; ++b) {
         unsigned long long pz;
-#ifdef VR_EXP_MORTON
-        const unsigned tz_ = wz[b] >> 3;
-        asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(pz) : "r"(tz_ >> 2), "r"(slab_bytes), "l"(vol_base));
-        const unsigned ez = (((tz_ & 2u) << 13) | ((tz_ & 1u) << 11) | ((wz[b] & 7) << 6)) + exc;
-#else
         asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(pz) : "r"(wz[b] >> 3), "r"(slab_bytes), "l"(vol_base));
         const unsigned ez = ((wz[b] & 7) << 6) + exc;
-#endif
 #pragma unroll
         for (int a = 0; a < 2; ++a)
             asm volatile("mad.wide.u32 %0, %1, 4, %2;" : "=l"(rp[a][b]) : "r"(ez + ey[a]), "l"(pz));
     }
     // byte distance from the chunk to voxel ix + 1 when ix is the chunk's last voxel: the next chunk of the same tile
     // row (16 B on) or, from a tile's second chunk, the first voxel of the next tile in x ((512 - 4) * 4 B on)
-#ifdef VR_EXP_MORTON
-    const unsigned de = (ix & 4u) ? (tile_fx((ix | 7u) + 1u) - tile_fx(ix & ~3u)) * 4u : 16u;
-#else
     const unsigned de = (ix & 4u) ? (TILE_ELEMS - 4) * 4u : 16u;
-#endif
 #pragma unroll
     for (int a = 0; a < 2; ++a)
 #pragma unroll

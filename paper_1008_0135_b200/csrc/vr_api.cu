@@ -1,4 +1,4 @@
-// vr_api.cu — the C ABI of include/vr.h: argument checks, per-frame planning on the host (plan.h)
+// vr_api.cu — the C ABI of include/vr.h (and the measurement aids of include/vr_measure.h): argument checks, per-frame planning on the host (plan.h)
 // and kernel launches (kernels.cuh).  Every step of the path runs in the kernels; this file only
 // validates, plans and enqueues.  There is no CPU fallback.
 #include <cuda_runtime.h>
@@ -13,9 +13,20 @@
 #include <vector>
 
 #include "../../include/vr.h"
+#include "../../include/vr_measure.h"
 #include "kernels.cuh"
 #include "slab.cuh"
 #include "plan.h"
+
+// Tuning constants of measurement builds (VR_DEFINES="-DVR_SEG_MAX=32" python -m paper_1008_0135_b200.build, which
+// writes a library file of its own; profiles/r02_experiments.md, r02_slab.md).  Product values:
+#ifndef VR_SEG_MAX
+#define VR_SEG_MAX 64        // samples per double-precision anchor, 1..64
+#endif
+#ifndef VR_SLAB_LOGD
+#define VR_SLAB_LOGD (-1)    // slab thickness chosen per frame
+#endif
+static_assert(VR_SEG_MAX >= 1 && VR_SEG_MAX <= 64 && VR_SLAB_LOGD >= -1 && VR_SLAB_LOGD <= 3, "tuning constants out of range");
 
 namespace {
 
@@ -71,8 +82,8 @@ struct vr_volume {
     // NEXT-2 empty-space skipping: occupancy mask (one bit per voxel cell), built for the current table on demand
     int n_runs = 0;                   // S2 channel mask as runs of enabled channels; 0 = every channel enabled
     int run_z[2 * vr::MAX_RUNS] = {0};
-    int pf_every = 0, pf_ahead = 0;   // experiment builds only (-DVR_EXP_L2PREFETCH): env VR_PF="every,ahead"
-    int seg_max = 64;                 // samples (and voxels of path) per anchored segment; env VR_SEG overrides (1..64)
+    int seg_max = VR_SEG_MAX;         // samples (and voxels of path) per anchored segment
+    bool debug = false;               // env VR_DEBUG=1 at vr_create_volume: wait for and check every kernel of a frame
     bool skip_enabled = true;
     unsigned long long* d_mask = nullptr;
     float* d_blockmax = nullptr;      // MIP skipping: largest voxel per block of 4x4x4 cells (same grid as the mask words)
@@ -86,7 +97,7 @@ struct vr_volume {
     long long mask_occupied = 0;
     // slab-staged caster (slab.cuh): linear padded copy, made on first use
     int slab_mode = 1;                // 0 off, 1 auto (dense orthographic frames), 2 whenever the window fits
-    int slab_logd = -1;               // env VR_SLAB_LOGD: force the slab thickness (tuning), -1 = heuristic
+    int slab_logd = VR_SLAB_LOGD;     // >= 0 forces the slab thickness 2^k cell layers (tuning builds), -1 = heuristic
     float* d_linear = nullptr;        // x fastest: views whose dominant axis is y or z
     float* d_linear_t = nullptr;      // z fastest: views whose dominant axis is x
     bool linear_failed = false;       // allocation failed once: stay on the row-cache caster
@@ -98,7 +109,7 @@ struct vr_volume {
 
 namespace {
 
-// element strides between tiles (product build) or macro-blocks (-DVR_EXP_MORTON) adjacent in y / z
+// element strides between tiles adjacent in y / z
 unsigned ty_stride_of(const vr_volume* v);
 unsigned slab_stride_of(const vr_volume* v);
 
@@ -110,13 +121,8 @@ struct Frame {                         // everything one frame needs, built on t
     size_t pool_pixels = 0;
 };
 
-#ifdef VR_EXP_MORTON
-unsigned ty_stride_of(const vr_volume* v) { return (unsigned)(v->TX / 4) * 32768u; }
-unsigned slab_stride_of(const vr_volume* v) { return (unsigned)(v->TX / 4) * (unsigned)(v->TY / 4) * 32768u; }
-#else
 unsigned ty_stride_of(const vr_volume* v) { return (unsigned)v->TX * vr::TILE_ELEMS; }
 unsigned slab_stride_of(const vr_volume* v) { return (unsigned)v->TX * (unsigned)v->TY * vr::TILE_ELEMS; }
-#endif
 
 vr_status check_render_args(const vr_volume* vol, const vr_camera* cam, int W, int H, float step, int mode) {
     if (!vol) return fail(VR_ERR_INVALID_ARG, "volume is NULL");
@@ -129,6 +135,14 @@ vr_status check_render_args(const vr_volume* vol, const vr_camera* cam, int W, i
                                   (double)vol->dims[2] * vol->dims[2]);
     if (diag / (double)step > 8.0e6) return fail(VR_ERR_INVALID_ARG, "step_voxels too small for this volume (> 8e6 samples per ray)");
     if (!vol->has_tf) return fail(VR_ERR_STATE, "no transfer function set (vr_set_transfer_function)");
+    return VR_OK;
+}
+
+// VR_DEBUG=1: wait for the kernel just launched and report its failure at the call that caused it (otherwise an
+// asynchronous fault surfaces at some later call).  Off by default: the frame path never synchronises.
+vr_status debug_sync(const vr_volume* vol, const char* what) {
+    if (!vol->debug) return VR_OK;
+    VR_CUDA(cudaStreamSynchronize(vol->stream), what);
     return VR_OK;
 }
 
@@ -170,7 +184,6 @@ vr_status build_frame(const vr_volume* vol, const vr_camera* cam, int W, int H, 
     P.seg_len = std::max(1, std::min(vol->seg_max, (int)((double)vol->seg_max / (double)step)));
     P.seg_span = (int)std::ceil((double)P.seg_len * (double)step) + 1;
     P.nbx = vol->NBX; P.nby = vol->NBY;
-    P.pf_every = vol->pf_every; P.pf_ahead = vol->pf_ahead;
     P.n_runs = vol->n_runs;
     for (int k = 0; k < 2 * vr::MAX_RUNS; ++k) P.run_z[k] = vol->run_z[k];
     P.x_zero_below = table_zero_below(vol);   // the per-step opacity correction keeps zeros zero
@@ -330,7 +343,7 @@ vr_status launch_cast(vr_volume* vol, const Frame& f, int mode, float* d_img, un
     }
 #undef VR_LAUNCH
     VR_CUDA(cudaGetLastError(), "cast kernel launch");
-    return VR_OK;
+    return debug_sync(vol, "cast kernel (VR_DEBUG)");
 }
 
 // ---- slab-staged caster (slab.cuh): eligibility, window sizing, tensor maps, launch ----
@@ -571,7 +584,7 @@ vr_status launch_slab_t(vr_volume* vol, const Frame& f, const SlabPlan& sp, floa
     vr::cast_slab_kernel<MODE, DOM><<<f.total_tiles, vr::CTA_THREADS, sp.smem, vol->stream>>>(
         f.P, sp.S, sp.maps, vol->d_bricks, (int)f.recs.size(), vol->d_tf_ea, d_img);
     VR_CUDA(cudaGetLastError(), "slab caster launch");
-    return VR_OK;
+    return debug_sync(vol, "slab caster (VR_DEBUG)");
 }
 
 vr_status launch_slab(vr_volume* vol, const Frame& f, const SlabPlan& sp, int mode, float* d_img) {
@@ -635,7 +648,7 @@ vr_status launch_composite(vr_volume* vol, const Frame& f, int mode, const float
         vr::composite_kernel<vr::MODE_MIP><<<grid, 256, 0, vol->stream>>>(vol->d_bricks, vol->d_order, B, d_img, W, H,
                                                                           vol->d_tf_raw, f.P.vmin, f.P.inv_range, d_out, d_scalar);
     VR_CUDA(cudaGetLastError(), "composite kernel launch");
-    return VR_OK;
+    return debug_sync(vol, "composite kernel (VR_DEBUG)");
 }
 
 // Brick images of vr_render live in one grow-only pool.  The rectangles change with the view, so the request is
@@ -665,28 +678,10 @@ vr_status vr_create_volume(const int dims[3], const float* d_data, vr_volume** o
     vr_volume* v = new (std::nothrow) vr_volume();
     if (!v) return fail(VR_ERR_OOM, "vr_create_volume: host allocation failed");
     for (int a = 0; a < 3; ++a) { v->dims[a] = dims[a]; v->sub_hi[a] = dims[a]; }
-    if (const char* pf = std::getenv("VR_PF")) {
-        int ev_ = 0, ah = 0;
-        if (std::sscanf(pf, "%d,%d", &ev_, &ah) == 2 && ev_ >= 0 && ev_ <= 64 && (ev_ & (ev_ - 1)) == 0 && ah >= 0 && ah <= 64) {
-            v->pf_every = ev_; v->pf_ahead = ah;
-        }
-    }
-    if (const char* e_ = std::getenv("VR_SLAB_LOGD")) {     // tuning knob: slab thickness 2^k cell layers
-        const int sv = std::atoi(e_);
-        if (sv >= 0 && sv <= 3) v->slab_logd = sv;
-    }
-    if (const char* e_ = std::getenv("VR_SEG")) {          // tuning knob for measurements
-        const int sv = std::atoi(e_);
-        if (sv >= 1 && sv <= 64) v->seg_max = sv;
-    }
+    if (const char* e_ = std::getenv("VR_DEBUG")) v->debug = e_[0] != '\0' && e_[0] != '0';   // the library's only environment variable
     // padded: PAD_a replicated layers below, at least one above
     v->TX = (dims[0] + vr::PAD_X + 1 + 7) / 8; v->TY = (dims[1] + vr::PAD_Y + 1 + 7) / 8; v->TZ = (dims[2] + vr::PAD_Z + 1 + 7) / 8;
-#ifdef VR_EXP_MORTON
-    v->TX = (v->TX + 3) & ~3; v->TY = (v->TY + 3) & ~3; v->TZ = (v->TZ + 3) & ~3;   // whole macro-blocks of 4x4x4 tiles
-    if ((double)v->TX * v->TY * 2048.0 >= 1073741824.0) {
-#else
     if ((double)v->TX * v->TY * vr::TILE_ELEMS >= 1073741824.0) {   // slab bytes and in-slab offsets stay 32-bit
-#endif
         delete v;
         return fail(VR_ERR_INVALID_ARG, "vr_create_volume: nx*ny too large for 32-bit in-slab offsets");
     }
@@ -1096,21 +1091,6 @@ vr_status vr_get_slab_info(const vr_volume* vol, int h_info[6], float* h_lineari
         const vr::LinearDims T = vr::linear_dims_t(vol->dims[0], vol->dims[1], vol->dims[2]);
         *h_linear_bytes = (vol->d_linear ? (long long)L.LX * L.LY * L.LZ * 4 : 0) + (vol->d_linear_t ? (long long)T.LX * T.LY * T.LZ * 4 : 0);
     }
-    return VR_OK;
-}
-
-vr_status vr_set_l2_fetch_granularity(int bytes) {
-    if (bytes != 32 && bytes != 64 && bytes != 128)
-        return fail(VR_ERR_INVALID_ARG, "vr_set_l2_fetch_granularity: bytes must be 32, 64 or 128");
-    VR_CUDA(cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)bytes), "cudaDeviceSetLimit(L2 fetch granularity)");
-    return VR_OK;
-}
-
-vr_status vr_get_l2_fetch_granularity(int* h_bytes) {
-    if (!h_bytes) return fail(VR_ERR_INVALID_ARG, "vr_get_l2_fetch_granularity: NULL argument");
-    size_t v = 0;
-    VR_CUDA(cudaDeviceGetLimit(&v, cudaLimitMaxL2FetchGranularity), "cudaDeviceGetLimit(L2 fetch granularity)");
-    *h_bytes = (int)v;
     return VR_OK;
 }
 

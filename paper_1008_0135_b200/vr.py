@@ -24,8 +24,8 @@ VR_MAX_CHANNEL_RUNS = 16
 SYMBOLS = ["vr_create_volume", "vr_destroy_volume", "vr_set_stream", "vr_set_transfer_function",
            "vr_set_bricks", "vr_set_subcube", "vr_set_channel_mask", "vr_render", "vr_render_to_host", "vr_render_to_host_async", "vr_wait_frames", "vr_render_bricks", "vr_composite",
            "vr_plan_bricks", "vr_measure", "vr_measure_units", "vr_set_empty_space_skipping", "vr_get_skip_info",
-           "vr_set_l2_fetch_granularity", "vr_set_slab_staging", "vr_get_slab_info", "vr_plan_slab",
-           "vr_get_l2_fetch_granularity", "vr_get_stage_ms", "vr_volume_info", "vr_volume_range", "vr_volume_histogram", "vr_volume_histogram_noalloc", "vr_export_linear", "vr_last_error"]
+           "vr_set_slab_staging", "vr_get_slab_info", "vr_plan_slab",
+           "vr_get_stage_ms", "vr_volume_info", "vr_volume_range", "vr_volume_histogram", "vr_volume_histogram_noalloc", "vr_export_linear", "vr_last_error"]
 
 
 class vr_camera(C.Structure):
@@ -73,11 +73,9 @@ def lib():
                                        C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
         L.vr_set_empty_space_skipping.argtypes = [vp, C.c_int]
         L.vr_get_skip_info.argtypes = [vp, ip, fp, C.POINTER(C.c_longlong), C.POINTER(C.c_double)]
-        L.vr_set_l2_fetch_granularity.argtypes = [C.c_int]
         L.vr_set_slab_staging.argtypes = [vp, C.c_int]
         L.vr_get_slab_info.argtypes = [vp, ip, fp, C.POINTER(C.c_longlong)]
         L.vr_plan_slab.argtypes = [ip, ip, cam, C.c_int, C.c_int, C.c_float, ip, C.POINTER(C.c_double), C.POINTER(C.c_double)]
-        L.vr_get_l2_fetch_granularity.argtypes = [ip]
         L.vr_get_stage_ms.argtypes = [vp, fp, fp]
         L.vr_volume_info.argtypes = [vp, fp, C.POINTER(C.c_longlong)]
         L.vr_volume_range.argtypes = [vp, fp, fp]
@@ -100,16 +98,6 @@ def vr_last_error():
 def _check(status):
     if status != VR_OK:
         raise VrError(status, vr_last_error())
-
-
-def vr_set_l2_fetch_granularity(nbytes):
-    _check(lib().vr_set_l2_fetch_granularity(int(nbytes)))
-
-
-def vr_get_l2_fetch_granularity():
-    v = C.c_int(0)
-    _check(lib().vr_get_l2_fetch_granularity(C.byref(v)))
-    return v.value
 
 
 def make_camera(view, projection, fovy_deg=45.0, ortho_half_h=1.0):

@@ -21,10 +21,13 @@ def vr():
     return binding
 
 
-def declared_symbols():
-    text = open(os.path.join(ROOT, "include", "vr.h")).read()
-    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(vr_[a-z0-9_]+)\s*\(", text)))
+def declared_symbols(headers=("vr.h", "vr_measure.h")):
+    names = set()
+    for h in headers:
+        text = open(os.path.join(ROOT, "include", h)).read()
+        text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+        names |= set(re.findall(r"\b(vr_[a-z0-9_]+)\s*\(", text))
+    return sorted(names)
 
 
 def test_header_symbols_exported(vr):
@@ -47,6 +50,16 @@ def test_experiment_builds_never_replace_the_product_library(monkeypatch):
     assert len({product, a, b}) == 3 and all(p.endswith(".so") for p in (a, b))
     names = {os.path.basename(p) for p in vr_build.deps()}
     assert {"vr_api.cu", "kernels.cuh", "sampler.cuh", "slab.cuh", "plan.h", "vr.h"} <= names
+
+
+def test_product_header_stays_small():
+    """include/vr.h is the product boundary (SURVEY.md section 8(b) + the NEXT rows); measurement and test aids live in
+    include/vr_measure.h."""
+    product = declared_symbols(("vr.h",))
+    aids = declared_symbols(("vr_measure.h",))
+    assert len(product) <= 24, product
+    assert set(aids) == {"vr_measure", "vr_measure_units", "vr_get_stage_ms", "vr_volume_info", "vr_export_linear"}
+    assert not set(product) & set(aids)
 
 
 def test_last_error_never_null(vr):
@@ -76,11 +89,9 @@ def test_null_and_range_checks_without_device(vr):
     assert L.vr_measure_units(None, C.byref(cam), 8, 8, 1.0, 0, 0.0, None, None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_set_empty_space_skipping(None, 1) == vr.VR_ERR_INVALID_ARG
     assert L.vr_get_skip_info(None, None, None, None, None) == vr.VR_ERR_INVALID_ARG
-    assert L.vr_set_l2_fetch_granularity(48) == vr.VR_ERR_INVALID_ARG
     assert L.vr_set_slab_staging(None, 1) == vr.VR_ERR_INVALID_ARG
     assert L.vr_get_slab_info(None, None, None, None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_plan_slab(None, None, C.byref(cam), 8, 8, 1.0, None, None, None) == vr.VR_ERR_INVALID_ARG
-    assert L.vr_get_l2_fetch_granularity(None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_volume_info(None, None, None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_export_linear(None, None) == vr.VR_ERR_INVALID_ARG
     assert L.vr_volume_range(None, None, None) == vr.VR_ERR_INVALID_ARG

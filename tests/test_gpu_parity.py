@@ -751,3 +751,24 @@ def test_render_to_host_async_delivers_the_same_frames(vr):
         vol.vr_render_to_host(cams[2], W, H, 0.5, 0, 0.0, one)
         assert torch.equal(one, want[2])
     vol.close()
+
+
+def test_debug_mode_renders_the_same_frame(vr, monkeypatch):
+    """VR_DEBUG=1 (read at vr_create_volume) waits for and checks every kernel of a frame; the frames are the same."""
+    import torch
+    w = wl.config(0)
+    cube = w.cube("cuda")
+    cs = wl.orbit_camera(w.dims, 40.0, 25.0, wl.PROJ_PERSP)
+    frames = []
+    for dbg in ("1", None):
+        if dbg is None:
+            monkeypatch.delenv("VR_DEBUG", raising=False)
+        else:
+            monkeypatch.setenv("VR_DEBUG", dbg)
+        vol = vr.Volume(cube)
+        vol.vr_set_transfer_function(w.table, w.vmin, w.vmax)
+        vol.vr_set_bricks(2, 2, 2)
+        frames.append(vol.vr_render(vr.camera_from_spec(cs), 96, 80, w.step, 0, 0.0).clone())
+        torch.cuda.synchronize()
+        vol.close()
+    assert torch.equal(frames[0], frames[1]) and float(frames[0][..., 3].max()) > 0.0
