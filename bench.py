@@ -35,14 +35,84 @@ from paper_1008_0135_b200 import workloads as wl
 
 METRIC = "ms_per_frame_1024x1024"
 UNIT = "ms/frame"
-# Per-launch DRAM traffic of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum of one
-# `ncu --set full` capture), keyed by the run it was captured on; any other run reports traffic = null.
-NCU_TRAFFIC = {
-    # (config, image, mode, bricks, skipping): (bytes per launch, profiles/ file the number comes from)
-    (3, 1024, 0, (2, 2, 2), True): (21.36e9, "profiles/r02_cast_full.md (skipping caster at the final HEAD, mean of launches az 10 / 20 deg, read + write)"),
-    (5, 1024, 0, (2, 2, 2), True): (5.14e9, "profiles/r02_slab.md (slab-staged caster on config 5, mean of launches az 0 / 10 deg, read + write)"),
-    (3, 1024, 0, (2, 2, 2), False): (27.23e9, "profiles/r02_cast_full.md (dense caster at the final HEAD, mean of launches az 10 / 20 deg, read + write)"),
-}
+# Per-launch DRAM traffic of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full`
+# capture) lives in profiles/traffic.csv, one row per captured run, written by `bench.py --record-traffic` from the
+# ncu CSV and stamped with a hash of paper_1008_0135_b200/csrc/.  A bench line carries the figure only when the row's
+# hash is the hash of the tree it runs on; after any kernel edit it reports traffic = null until re-captured.
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "traffic.csv")
+TRAFFIC_FIELDS = ["config", "image", "mode", "bricks", "skipping", "kernel", "bytes_per_launch", "launches", "csrc_sha256",
+                  "captured_after_commit", "source"]
+
+
+def csrc_hash():
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    for p in sorted(glob.glob(os.path.join(ROOT, "paper_1008_0135_b200", "csrc", "*"))):
+        h.update(os.path.basename(p).encode() + b"\0")
+        with open(p, "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
+def traffic_key(config, W, H, mode, bricks, skipping):
+    return (str(config), str(W if W == H else -1), str(mode), "x".join(str(b) for b in bricks), "1" if skipping else "0")
+
+
+def read_traffic(key):
+    """(bytes per launch or None, text saying where the figure comes from or why there is none)."""
+    import csv
+    if not os.path.exists(TRAFFIC_CSV):
+        return None, "no profiles/traffic.csv"
+    tree = csrc_hash()
+    stale = None
+    with open(TRAFFIC_CSV, newline="") as f:
+        for row in csv.DictReader(f):
+            if (row["config"], row["image"], row["mode"], row["bricks"], row["skipping"]) != key:
+                continue
+            if row["csrc_sha256"] == tree:
+                return float(row["bytes_per_launch"]), f"{row['source']} ({row['kernel']}, mean of {row['launches']} launches, csrc {tree})"
+            stale = f"stale: profiles/traffic.csv holds a capture of csrc {row['csrc_sha256']}, this tree is {tree} (re-capture and --record-traffic)"
+    return None, stale or "this run was never captured under ncu"
+
+
+def record_traffic(args):
+    """bench.py --record-traffic NCU.csv --traffic-source profiles/x.md [--config N --no-skip --image S]: NCU.csv is
+    `ncu -i REPORT.ncu-rep --page raw --csv --print-units base` of a capture of THIS bench command on THIS tree."""
+    import csv
+    with open(args.record_traffic, newline="") as f:
+        rows = [r for r in csv.reader(f) if r]
+    head = next(k for k, r in enumerate(rows) if "Kernel Name" in r)
+    h = rows[head]
+    kn, rd, wr = h.index("Kernel Name"), h.index("dram__bytes_read.sum"), h.index("dram__bytes_write.sum")
+    per = {}
+    for r in rows[head + 1:]:
+        try:
+            b = float(r[rd].replace(",", "")) + float(r[wr].replace(",", ""))
+        except (ValueError, IndexError):
+            continue                                              # the units row
+        name = r[kn].split("(")[0]
+        if "cast" in name:
+            per.setdefault(name, []).append(b)
+    if not per:
+        raise SystemExit("bench.py --record-traffic: no caster launch in " + args.record_traffic)
+    kernel = max(per, key=lambda k: sum(per[k]))                  # the dominant caster of the capture
+    w, _ = workload_for(args)
+    skipping = (not args.no_skip) and w.mode == 0
+    key = traffic_key(args.config, w.W, w.H, w.mode, w.bricks, skipping)
+    commit = subprocess.run(["git", "rev-parse", "--short", "HEAD"], cwd=ROOT, capture_output=True, text=True).stdout.strip()
+    new = dict(zip(TRAFFIC_FIELDS, list(key) + [kernel, f"{sum(per[kernel]) / len(per[kernel]):.0f}", str(len(per[kernel])),
+                                                csrc_hash(), commit, args.traffic_source or args.record_traffic]))
+    old = []
+    if os.path.exists(TRAFFIC_CSV):
+        with open(TRAFFIC_CSV, newline="") as f:
+            old = [r for r in csv.DictReader(f) if tuple(r[k] for k in TRAFFIC_FIELDS[:5]) != key]
+    with open(TRAFFIC_CSV, "w", newline="") as f:
+        wtr = csv.DictWriter(f, fieldnames=TRAFFIC_FIELDS)
+        wtr.writeheader()
+        for r in old + [new]:
+            wtr.writerow(r)
+    print(json.dumps(new))
 
 
 def env_int(name, default):
@@ -215,8 +285,6 @@ def run_ours(args):
 
     w, views = workload_for(args)
     K, Wm = args.steps, args.warmup
-    if args.l2_fetch:
-        vr.vr_set_l2_fetch_granularity(args.l2_fetch)
     cube = w.cube("cuda")
     torch.cuda.synchronize()
     vol = vr.Volume(cube)
@@ -375,8 +443,7 @@ def run_ours(args):
                   "gate": 5e-3 if w.ert_alpha > 0 else 1e-4}
         del host_cube
 
-    traffic, traffic_src = NCU_TRAFFIC.get((args.config, w.W if w.W == w.H else -1, w.mode, tuple(w.bricks),
-                                            bool(skip_info["active"])), (None, None))
+    traffic, traffic_src = read_traffic(traffic_key(args.config, w.W, w.H, w.mode, w.bricks, bool(skip_info["active"])))
     cfg = describe(w, views)
     cfg["views_timed"] = {"count": len(used_views), "azimuths_deg": [views[v] for v in used_views],
                           "note": "view k of the timed region is azimuth views[k mod len(views)]; steps < len(views) time a prefix of the orbit"}
@@ -579,10 +646,14 @@ def main():
                     help="with --sweep: run only the points matching MODE:BRICKS:STEP:SIZE (e.g. EA:8:0.25:2048; * = any)")
     ap.add_argument("--slab", type=int, default=None, choices=[0, 1, 2],
                     help="vr_set_slab_staging: 0 never, 1 auto (library default), 2 whenever the window fits")
-    ap.add_argument("--l2-fetch", type=int, default=None, choices=[32, 64, 128],
-                    help="device-wide L2 fetch granularity hint in bytes (vr_set_l2_fetch_granularity); default: leave as is")
     ap.add_argument("--sweep", action="store_true", help="run BASELINE.json configs[4] (28 points) instead of the headline")
+    ap.add_argument("--record-traffic", default=None, metavar="NCU_CSV",
+                    help="no benchmark: store the caster's mean DRAM bytes per launch of an ncu raw CSV in profiles/traffic.csv")
+    ap.add_argument("--traffic-source", default=None, help="with --record-traffic: the profiles/ file that describes the capture")
     args = ap.parse_args()
+    if args.record_traffic:
+        record_traffic(args)
+        return
     launch_ranks_if_needed(args)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.cpu_stride is None:
